@@ -1,0 +1,316 @@
+#!/usr/bin/env python
+"""bench.py — cell-updates/s of the fused MUSCL-Hancock + Roe step on B200, with roofline.
+
+One "step" = one pass of the whole hot path (reconstruction, half-step prediction, Roe solver, full-step
+update, boundary fluxes) over one batch of synthetic patch groups. At N = 1 the workload is
+BASELINE.json:configs[3], the configuration the metric is quoted on: 32768 groups of 16^3 cells (+2 ghost
+layers) cut from a seeded 512^3 cosmology-like baryonic field, fp32, gamma = 5/3, MinMod, one step per
+launch. With N > 1 (torchrun, one rank per GPU) every rank owns its own 32768-group batch (seed + rank):
+patch groups are independent, so the path shards with no collective ("scaling": "weak").
+
+Contract: `python bench.py --gpus N --steps K --warmup W [--impl reference]` prints ONE JSON line on rank 0.
+  value      whole-job cell-updates/s with inputs resident in HBM (CUDA events, max over ranks)
+  e2e        same metric through the C-ABI host-buffer call gamer_hydro_step_host (pinned host memory,
+             H2D + kernels + D2H inside the timed region)
+  roofline   ALU-bound: counted algorithmic FLOPs (the oracle's CountingReal tally) / time
+             against 148 SM x 128 lanes x 2 x 1.965 GHz; the HBM side is reported next to it
+  cpu_baseline  the fp64 oracle as it stands, on this box's host cores, on a bounded sample of the same
+             workload (rank 0, N = 1 only); the same sample doubles as a parity spot-check
+`--impl reference` times the oracle alone (this tier's reference arm).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "cell-updates/s (fp32 MUSCL-Hancock+Roe step, 16^3 patch groups with 2-cell ghost shell)"
+UNIT = "cell-updates/s"
+N, GHOST = 16, 2
+# algorithmic FLOPs per cell-update: oracle CountingReal tally on an all-slopes-active field (
+# tests/test_oracle_pins.py::test_flop_tally_band re-derives it). Hand count of SURVEY.md App. D: 925 / 966.
+FLOPS_PER_CELL = {0: 1033.94, 1: 1095.81}
+BYTES_PER_CELL = 66.5625           # (5*20^3 + 5*16^3 + 30*16^2) * 4 B / 16^3
+SM_COUNT, LANES, SM_MAX_GHZ = 148, 128, 1.965
+ALU_PEAK_TFLOPS = SM_COUNT * LANES * 2 * SM_MAX_GHZ / 1e3     # 74.45
+
+
+def measured_hbm_peak():
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.stop_flag = [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown",
+                 nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def result(self):
+        self.stop_flag = True
+        if self.is_alive():
+            self.join()
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": ["nvml unavailable"]}
+        return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.samples)}
+
+
+def make_workload(n_box, seed):
+    from paper_1007_3818_b200 import workloads as wl
+    t0 = time.time()
+    w = wl.config_3_cosmo(n_box, seed=seed)
+    groups = w.groups(np.float32)
+    dt = w.dt()
+    dx = float(np.float32(w.dx))
+    return w, groups, dt, dx, time.time() - t0
+
+
+def run_reference(args, rank, world):
+    """This tier's reference arm: the fp64 oracle alone, on the host cores, on a bounded sample per step."""
+    if rank != 0:
+        return
+    from oracle import mhm_oracle as O
+    w, groups, dt, dx, _ = make_workload(64, args.seed)      # 64 groups of the same recipe: a bounded sample
+    sample = groups[: args.ref_groups]
+    for _ in range(args.warmup):
+        O.step_groups(sample, N, GHOST, dt, dx, w.gamma, w.limiter, want_guard=False)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r = O.step_groups(sample, N, GHOST, dt, dx, w.gamma, w.limiter, want_guard=False)
+    t = time.perf_counter() - t0
+    cells = sample.shape[0] * N ** 3 * args.steps
+    val = cells / t
+    desc = "%d groups of the cfg3 recipe (64^3 box) per step, all host cores" % sample.shape[0]
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "cfg3_cosmo (BASELINE.json:configs[3]) bounded sample: " + desc,
+                   "limiter": "minmod", "gamma": w.gamma},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": r.threads, "kind": "oracle", "sample": desc},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0}))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--box", type=int, default=512, help="global box edge; 512 -> 32768 groups (headline)")
+    ap.add_argument("--seed", type=int, default=3)
+    ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--cpu-groups", type=int, default=192, help="groups in the oracle sample (cpu_baseline)")
+    ap.add_argument("--ref-groups", type=int, default=64)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+
+    import torch
+    import torch.distributed as dist
+    import paper_1007_3818_b200 as gh
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    w, groups, dt, dx, gen_s = make_workload(args.box, args.seed + rank)
+    G = groups.shape[0]
+    cells = G * N ** 3
+    gh.gamer_hydro_alloc(G, N, GHOST, 4, local_rank)
+    h_in = torch.from_numpy(groups)
+    d_in = h_in.to(dev)
+    d_out = torch.empty((G, 5, N, N, N), dtype=torch.float32, device=dev)
+    d_bf = torch.empty((G, 6, 5, N, N), dtype=torch.float32, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        gh.gamer_hydro_step(d_in, d_out, d_bf, G, N, GHOST, dt, dx, w.gamma, w.limiter, stream=stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    barrier()
+    gh.gamer_hydro_status()                                   # reset the diagnostics counters
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    launches0 = gh.gamer_hydro_launch_count()
+    barrier()
+    evs[0].record(stream)
+    for s in range(args.steps):
+        step()
+        evs[s + 1].record(stream)
+    barrier()
+    clocks = sampler.result()
+    launches = gh.gamer_hydro_launch_count() - launches0
+    total_ms = evs[0].elapsed_time(evs[-1])
+    per_step = [evs[s].elapsed_time(evs[s + 1]) for s in range(args.steps)]
+    guard_cells, nonpos = gh.gamer_hydro_status()
+    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    total_ms_max = float(tmax.item())
+    value = world * cells * args.steps / (total_ms_max * 1e-3)
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hp_in = h_in.pin_memory()
+        hp_out = torch.empty((G, 5, N, N, N), dtype=torch.float32).pin_memory()
+        hp_bf = torch.empty((G, 6, 5, N, N), dtype=torch.float32).pin_memory()
+
+        def e2e_step():
+            gh.gamer_hydro_step_host(hp_in, hp_out, hp_bf, G, N, GHOST, dt, dx, w.gamma, w.limiter, chunk_groups=0)
+
+        e2e_step()
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.e2e_steps):
+            e2e_step()
+        barrier()
+        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * cells * args.e2e_steps / float(te.item()), "unit": UNIT,
+               "h2d_bytes_per_step": int(hp_in.numel() * 4),
+               "d2h_bytes_per_step": int((hp_out.numel() + hp_bf.numel()) * 4),
+               "steps": args.e2e_steps, "api": "gamer_hydro_step_host (pinned host buffers, chunked 3-stream overlap)"}
+        same = bool(torch.equal(hp_out, d_out.cpu()))
+        e2e["matches_device_path_bitwise"] = same
+        del hp_in, hp_out, hp_bf
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant (only) kernel: fused_kernel<float, MinMod>
+    ms_launch = total_ms / args.steps                         # one launch per step on this rank
+    flops = FLOPS_PER_CELL[w.limiter] * cells
+    achieved_tf = flops / (ms_launch * 1e-3) / 1e12
+    hbm_peak, hbm_src = measured_hbm_peak()
+    hbm_gbs = BYTES_PER_CELL * cells / (ms_launch * 1e-3) / 1e9
+    traffic = None
+    try:
+        with open(os.path.join(ROOT, "profiles", "traffic_bytes_per_launch.json")) as f:
+            tj = json.load(f)
+            if tj.get("n_groups") == G:
+                traffic = tj["dram_bytes_read_plus_write"]
+    except Exception:
+        pass
+    roofline = {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                "frac": achieved_tf / ALU_PEAK_TFLOPS, "traffic": traffic,
+                "kernel": "gh::fused_kernel<float, MinMod>",
+                "flops_per_cell_update": FLOPS_PER_CELL[w.limiter],
+                "peak_derivation": "148 SM x 128 FP32 lanes x 2 FLOP x 1.965 GHz (sm_max_mhz of MEASURED_PEAKS.json)",
+                "ms_per_launch": ms_launch,
+                "hbm": {"algorithmic_bytes_per_launch": BYTES_PER_CELL * cells, "achieved_gbs": hbm_gbs,
+                        "peak_gbs": hbm_peak, "peak_source": hbm_src, "frac": hbm_gbs / hbm_peak},
+                "frac_of_binding_roofline_time": max(flops / (ALU_PEAK_TFLOPS * 1e12),
+                                                     BYTES_PER_CELL * cells / (hbm_peak * 1e9)) / (ms_launch * 1e-3)}
+
+    # ---- cpu_baseline: the oracle on a bounded sample of the same workload (+ parity spot-check)
+    cpu = None
+    if not args.no_cpu_baseline and world == 1:
+        from oracle import mhm_oracle as O
+        sys.path.insert(0, os.path.join(ROOT, "tests"))
+        import metrics
+        import parity_util as pu
+        rng = np.random.default_rng(12345)
+        rho_max = groups[:, 0, 2:-2, 2:-2, 2:-2].reshape(G, -1).max(axis=1)
+        pick = set(int(i) for i in rng.choice(G, size=min(args.cpu_groups, G) - 2, replace=False))
+        pick.update([int(np.argmax(rho_max)), int(np.argmin(rho_max))])
+        idx = np.array(sorted(pick))
+        sample = np.ascontiguousarray(groups[idx])
+        t0 = time.perf_counter()
+        r = O.step_groups(sample, N, GHOST, dt, dx, w.gamma, w.limiter)
+        tc = time.perf_counter() - t0
+        gout = d_out[torch.from_numpy(idx).to(dev)].cpu().numpy()
+        sus = pu.suspect_mask(r.margin)
+        err = metrics.max_rel_err(gout, r.U_out, w.gamma, mask=np.broadcast_to(~sus[:, None], r.U_out.shape))
+        desc = "%d of the %d groups (seeded random + the groups holding max/min density), one step" % (len(idx), G)
+        cpu = {"value": len(idx) * N ** 3 / tc, "unit": UNIT, "cores": r.threads, "kind": "oracle", "sample": desc,
+               "seconds": tc, "parity_max_rel_err_on_sample": err, "parity_tolerance": 1e-4,
+               "parity_excluded_fraction": float(sus.mean()), "oracle_guard_cells_on_sample": r.guard_cells}
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
+           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "config": {"workload": "cfg3_cosmo_%d (BASELINE.json:configs[3]): %d patch groups/GPU, 16^3+2 ghost, "
+                                  "5 vars, gamma=5/3, MinMod, 1 step per launch" % (args.box, G),
+                      "groups_per_gpu": G, "cells_per_gpu": cells, "seed": args.seed,
+                      "l2": "inputs (%.2f GB/step) far larger than the 126 MB L2; no flush needed" %
+                            (h_in.numel() * 4 / 1e9),
+                      "parallelism": "groups sharded across ranks, no collective",
+                      "generation_seconds": gen_s, "dt": dt, "dx": dx},
+           "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
+           "clocks": clocks, "ms_per_step_min": min(per_step), "ms_per_step_median": float(np.median(per_step)),
+           "guard_cells_per_step": guard_cells / args.steps, "nonpositive_out_per_step": nonpos / args.steps,
+           "context_paper": {"gpu_vs_cpu_solver_speedup": 55.0, "overall_speedup_8800GTX": 19.2,
+                             "overall_speedup_T10_rtvd": 16.5, "source": "PAPER.md:27,29,13 (other hardware)"}}
+    print(json.dumps(out))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

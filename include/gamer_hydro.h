@@ -1,0 +1,99 @@
+/* include/gamer_hydro.h — C ABI of the B200-native GAMER hydro hot path (arXiv 1007.3818).
+ *
+ * What the library computes. PAPER.md:15 (§2): "a new GPU hydrodynamic solver based on the MUSCL-Hancock
+ * method. This approach contains four steps, namely, the spatial data reconstruction, the half-step
+ * prediction, the Riemann solver, and the full-step update. We apply the unsplit finite volume method for
+ * the three-dimensional evolution, and the Roe's solver is adopted for the Riemann problem."
+ * PAPER.md:27 (§2): "it requires only a five-point stencil in each spatial direction" (=> 2 ghost cells) and
+ * "the operation of preparing the ghost-zone data is conducted by CPU": the caller hands over a batch of
+ * patch groups WITH their ghost shells already filled; one call advances every group by one time step.
+ * The numerical details the paper leaves open are fixed in DESIGN.md §3 (readings R1–R21).
+ *
+ * All functions: extern "C", never throw, never exit; return 0 on success or a GAMER_HYDRO_* code.
+ * Pointers are DEVICE pointers unless the name says host. Nothing here takes or returns a torch type.
+ *
+ * Layouts (x fastest, then y, then z; `real` = float or double):
+ *   U_in            real[n_groups][5][S][S][S],  S = N + 2*ghost; variables (rho, mx, my, mz, E);
+ *                   interior cell (i,j,k) sits at (i+ghost, j+ghost, k+ghost). Only the innermost two ghost
+ *                   layers are read; of those, corner ghosts and layer-2 edge ghosts are never read.
+ *   U_out           real[n_groups][5][N][N][N]
+ *   boundary_fluxes real[n_groups][6][5][N][N] or NULL (skipped). Faces ordered -x,+x,-y,+y,-z,+z (face index
+ *                   -1/2 and N-1/2 along the axis); in-face index [k][j] for x faces, [k][i] for y faces,
+ *                   [j][i] for z faces. Each entry is the Roe flux DENSITY ALONG THE +AXIS (not the outward
+ *                   normal) of (rho, mx, my, mz, E), exactly the value used in the update.
+ * Ownership: the caller owns every buffer; the library never allocates, frees or keeps them. U_in is
+ * read-only; outputs must not alias U_in. Device pointers must be 16-byte aligned.
+ * Equation of state: ideal gas, E = P/(gamma-1) + rho |v|^2 / 2.  limiter: 0 = MinMod, 1 = van Leer.
+ */
+#ifndef GAMER_HYDRO_H
+#define GAMER_HYDRO_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct CUstream_st* cudaStream_t;
+
+enum {
+  GAMER_HYDRO_OK = 0,
+  GAMER_HYDRO_INVALID_ARG = 1, /* null U_in/U_out, n_groups<0, N<1, ghost<2, dt/dx not finite or <=0, gamma<=1,
+                                  unknown limiter, misaligned pointer */
+  GAMER_HYDRO_UNSUPPORTED = 2, /* shape the library has no kernel for */
+  GAMER_HYDRO_CUDA_ERROR = 3,  /* a CUDA call failed; gamer_hydro_strerror(3) carries the CUDA message */
+  GAMER_HYDRO_NOT_SM100 = 4    /* the device is not compute capability 10.x */
+};
+
+enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1 };
+
+/* kernel selection for gamer_hydro_set_path: AUTO picks FUSED when N == 16, else GENERIC */
+enum { GAMER_HYDRO_PATH_AUTO = 0, GAMER_HYDRO_PATH_GENERIC = 1, GAMER_HYDRO_PATH_FUSED = 2 };
+
+/* One-time, idempotent, process-global set-up for `device`: checks the compute capability, raises the
+ * dynamic shared-memory limits of the kernels, allocates the device status block and (for the generic
+ * path and the host-buffer path) scratch sized for min(max_groups, internal chunk) groups of N^3 cells
+ * with `bytes_per_real` (4 or 8). Synchronous. gamer_hydro_step* call it with defaults when it was not
+ * called. Calling it again with larger sizes grows the scratch. */
+int gamer_hydro_alloc(int max_groups, int N, int ghost, int bytes_per_real, int device);
+
+/* Releases everything gamer_hydro_alloc created (synchronises the device first). */
+void gamer_hydro_free(void);
+
+/* One MUSCL-Hancock + Roe time step on n_groups patch groups, fp32. Enqueues on `stream` and
+ * returns without synchronising; re-entrant across streams. Deterministic: each cell's arithmetic sequence
+ * is fixed, so results do not depend on n_groups or on the launch geometry. n_groups == 0 is a no-op.
+ * Non-positive rho or P in the input is the caller's fault: no hang, garbage confined to that group.
+ * This is the signature fixed by BASELINE.json:north_star. */
+int gamer_hydro_step(const float* U_in_with_ghosts, float* U_out, float* boundary_fluxes, int n_groups, int N,
+                     int ghost, float dt, float dx, float gamma, int limiter, cudaStream_t stream);
+
+/* Same step in fp64 (parity target 1e-11 against the fp64 oracle). */
+int gamer_hydro_step_f64(const double* U_in_with_ghosts, double* U_out, double* boundary_fluxes, int n_groups,
+                         int N, int ghost, double dt, double dx, double gamma, int limiter, cudaStream_t stream);
+
+/* Same fp32 step with HOST buffers (pinned memory recommended; pageable works but serialises the copies).
+ * The batch is streamed through the device in chunks: H2D copy, kernel and D2H copy of consecutive chunks
+ * overlap on internal streams — the B200 counterpart of the paper's overlap of data transfer with
+ * computation ("concurrent execution between CPU and GPU"). Synchronous: returns
+ * when U_out / boundary_fluxes (host) are complete. chunk_groups <= 0 picks the default. */
+int gamer_hydro_step_host(const float* h_U_in_with_ghosts, float* h_U_out, float* h_boundary_fluxes, int n_groups,
+                          int N, int ghost, float dt, float dx, float gamma, int limiter, int chunk_groups);
+
+/* Diagnostics accumulated since the last call (and reset by it): number of cells whose predicted face
+ * states failed the positivity guard and fell back to first order (R7), and number of updated
+ * cells with rho <= 0 or P <= 0 (R10: counted, never floored). Synchronises the device. Either pointer may
+ * be NULL. */
+int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonpositive_out);
+
+/* Forces a kernel path (tests, benchmarking); GAMER_HYDRO_PATH_AUTO restores the default. */
+int gamer_hydro_set_path(int path);
+
+/* Number of kernel launches the library has enqueued since it was loaded (bench.py's gpu_launches). */
+unsigned long long gamer_hydro_launch_count(void);
+
+/* Static string for a return code; for GAMER_HYDRO_CUDA_ERROR the last CUDA error message. */
+const char* gamer_hydro_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GAMER_HYDRO_H */

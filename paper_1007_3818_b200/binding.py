@@ -1,0 +1,132 @@
+"""Thin Python face of the C ABI in include/gamer_hydro.h — argument marshalling only. Every step of the hot
+path (reconstruction, half-step prediction, Roe solver, full-step update) runs inside
+libgamer_hydro.so's CUDA kernels; PyTorch supplies device memory and streams, nothing else. There is no CPU
+fallback: if the library is missing or no sm_100 device is present the calls raise.
+
+Function names and argument order follow the C header one to one.
+"""
+import ctypes as C
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libgamer_hydro.so")
+_lib = None
+
+MINMOD, VANLEER = 0, 1
+PATH_AUTO, PATH_GENERIC, PATH_FUSED = 0, 1, 2
+
+EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
+           "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
+           "gamer_hydro_strerror"]
+
+
+class GamerHydroError(RuntimeError):
+    pass
+
+
+def lib():
+    """Loads libgamer_hydro.so (built in-tree by paper_1007_3818_b200/build.py). Fails loudly when absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise GamerHydroError("CUDA extension %s is missing: run `python -c 'import __graft_entry__ as g; "
+                                  "g.build()'` (no CPU fallback exists)" % _LIB_PATH)
+        L = C.CDLL(_LIB_PATH)
+        vp, i, f, d = C.c_void_p, C.c_int, C.c_float, C.c_double
+        L.gamer_hydro_alloc.argtypes = [i, i, i, i, i]
+        L.gamer_hydro_free.restype = None
+        L.gamer_hydro_step.argtypes = [vp, vp, vp, i, i, i, f, f, f, i, vp]
+        L.gamer_hydro_step_f64.argtypes = [vp, vp, vp, i, i, i, d, d, d, i, vp]
+        L.gamer_hydro_step_host.argtypes = [vp, vp, vp, i, i, i, f, f, f, i, i]
+        L.gamer_hydro_status.argtypes = [C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
+        L.gamer_hydro_set_path.argtypes = [i]
+        L.gamer_hydro_launch_count.restype = C.c_ulonglong
+        L.gamer_hydro_strerror.restype = C.c_char_p
+        L.gamer_hydro_strerror.argtypes = [i]
+        _lib = L
+    return _lib
+
+
+def gamer_hydro_strerror(code):
+    return lib().gamer_hydro_strerror(int(code)).decode()
+
+
+def _check(rc):
+    if rc != 0:
+        raise GamerHydroError("gamer_hydro error %d: %s" % (rc, gamer_hydro_strerror(rc)))
+
+
+def gamer_hydro_alloc(max_groups, N=16, ghost=2, bytes_per_real=4, device=0):
+    _check(lib().gamer_hydro_alloc(int(max_groups), int(N), int(ghost), int(bytes_per_real), int(device)))
+
+
+def gamer_hydro_free():
+    lib().gamer_hydro_free()
+
+
+def _stream_ptr(stream):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+def _shapes(U_in, N, ghost):
+    S = N + 2 * ghost
+    if U_in.dim() != 5 or tuple(U_in.shape[1:]) != (5, S, S, S):
+        raise GamerHydroError("U_in must be [n_groups][5][%d][%d][%d], got %s" % (S, S, S, tuple(U_in.shape)))
+    return U_in.shape[0]
+
+
+def _step(fn, dtype, U_in, U_out, boundary_fluxes, N, ghost, dt, dx, gamma, limiter, stream):
+    G = _shapes(U_in, N, ghost)
+    for x in (U_in, U_out, boundary_fluxes):
+        if x is not None and not (x.is_cuda and x.dtype == dtype and x.is_contiguous()):
+            raise GamerHydroError("tensors must be contiguous CUDA tensors of dtype %s" % dtype)
+    if U_out is None:
+        U_out = torch.empty((G, 5, N, N, N), dtype=dtype, device=U_in.device)
+    bf = boundary_fluxes.data_ptr() if boundary_fluxes is not None else None
+    _check(fn(U_in.data_ptr(), U_out.data_ptr(), bf, G, N, ghost, dt, dx, gamma, int(limiter), _stream_ptr(stream)))
+    return U_out
+
+
+def gamer_hydro_step(U_in_with_ghosts, U_out, boundary_fluxes, n_groups=None, N=16, ghost=2, dt=None, dx=None,
+                     gamma=5.0 / 3.0, limiter=MINMOD, stream=None):
+    """fp32 step on device tensors; enqueues on `stream` (default: torch's current stream) and returns U_out."""
+    assert n_groups is None or n_groups == U_in_with_ghosts.shape[0]
+    return _step(lib().gamer_hydro_step, torch.float32, U_in_with_ghosts, U_out, boundary_fluxes, N, ghost, dt, dx,
+                 gamma, limiter, stream)
+
+
+def gamer_hydro_step_f64(U_in_with_ghosts, U_out, boundary_fluxes, n_groups=None, N=16, ghost=2, dt=None, dx=None,
+                         gamma=5.0 / 3.0, limiter=MINMOD, stream=None):
+    assert n_groups is None or n_groups == U_in_with_ghosts.shape[0]
+    return _step(lib().gamer_hydro_step_f64, torch.float64, U_in_with_ghosts, U_out, boundary_fluxes, N, ghost, dt,
+                 dx, gamma, limiter, stream)
+
+
+def gamer_hydro_step_host(h_U_in, h_U_out, h_boundary_fluxes, n_groups=None, N=16, ghost=2, dt=None, dx=None,
+                          gamma=5.0 / 3.0, limiter=MINMOD, chunk_groups=0):
+    """fp32 step on HOST tensors (pinned recommended); copies are inside the call; synchronous."""
+    G = _shapes(h_U_in, N, ghost)
+    for x in (h_U_in, h_U_out, h_boundary_fluxes):
+        if x is not None and (x.is_cuda or x.dtype != torch.float32 or not x.is_contiguous()):
+            raise GamerHydroError("host tensors must be contiguous CPU float32 tensors")
+    bf = h_boundary_fluxes.data_ptr() if h_boundary_fluxes is not None else None
+    _check(lib().gamer_hydro_step_host(h_U_in.data_ptr(), h_U_out.data_ptr(), bf, G, N, ghost, dt, dx, gamma,
+                                       int(limiter), int(chunk_groups)))
+    return h_U_out
+
+
+def gamer_hydro_status():
+    a, b = C.c_ulonglong(0), C.c_ulonglong(0)
+    _check(lib().gamer_hydro_status(C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
+
+
+def gamer_hydro_set_path(path):
+    _check(lib().gamer_hydro_set_path(int(path)))
+
+
+def gamer_hydro_launch_count():
+    return int(lib().gamer_hydro_launch_count())

@@ -1,0 +1,358 @@
+// csrc/gamer_hydro_api.cu — the C ABI declared in include/gamer_hydro.h: argument validation, TMA descriptor
+// encoding, kernel selection and launch. No torch types, no CPU fallback: without a compute-capability-10
+// device every compute entry point returns an error.
+#include <cuda.h>
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <atomic>
+#include <mutex>
+
+#include "../../include/gamer_hydro.h"
+#include "hydro_fused.cuh"
+#include "hydro_generic.cuh"
+
+namespace {
+
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+struct State {
+  bool ready = false;
+  int device = -1;
+  int sm_count = 0;
+  unsigned long long* status = nullptr;  // [0] guard cells, [1] non-positive outputs
+  void* scratch = nullptr;               // generic path: FS + FL for `scratch_groups` groups
+  size_t scratch_bytes = 0;
+  // host-buffer path
+  cudaStream_t hstream[3] = {nullptr, nullptr, nullptr};
+  void* hbuf_in[3] = {nullptr, nullptr, nullptr};
+  void* hbuf_out[3] = {nullptr, nullptr, nullptr};
+  void* hbuf_bf[3] = {nullptr, nullptr, nullptr};
+  size_t hbuf_groups = 0;
+  int hbuf_N = 0, hbuf_ghost = 0;
+  int path = GAMER_HYDRO_PATH_AUTO;
+  char cuda_msg[256] = "no CUDA error recorded";
+  EncodeTiledFn encode = nullptr;
+};
+
+State g_state;
+std::mutex g_mutex;
+std::atomic<unsigned long long> g_launches{0};
+
+constexpr int kGenericChunk = 512;  // groups per generic-path launch (bounds the scratch buffer)
+
+int cuda_fail(cudaError_t e, const char* what) {
+  snprintf(g_state.cuda_msg, sizeof(g_state.cuda_msg), "%s: %s", what, cudaGetErrorString(e));
+  return GAMER_HYDRO_CUDA_ERROR;
+}
+#define CK(call)                                        \
+  do {                                                  \
+    cudaError_t e_ = (call);                            \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #call); \
+  } while (0)
+
+template <class R, int LIM, bool Fast>
+int set_fused_attr() {
+  CK(cudaFuncSetAttribute(gh::fused_kernel<R, LIM, Fast>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                          gh::FusedSmem<R>::total));
+  return 0;
+}
+
+int init_locked(int device) {
+  if (g_state.ready && g_state.device == device) return 0;
+  if (g_state.ready) return GAMER_HYDRO_INVALID_ARG;  // one device per process
+  int count = 0;
+  CK(cudaGetDeviceCount(&count));
+  if (device < 0 || device >= count) return GAMER_HYDRO_INVALID_ARG;
+  cudaDeviceProp prop;
+  CK(cudaGetDeviceProperties(&prop, device));
+  if (prop.major != 10) return GAMER_HYDRO_NOT_SM100;
+  CK(cudaSetDevice(device));
+  g_state.sm_count = prop.multiProcessorCount;
+  CK(cudaMalloc(&g_state.status, 2 * sizeof(unsigned long long)));
+  CK(cudaMemset(g_state.status, 0, 2 * sizeof(unsigned long long)));
+  int rc;
+  if ((rc = set_fused_attr<float, 0, true>())) return rc;
+  if ((rc = set_fused_attr<float, 1, true>())) return rc;
+  if ((rc = set_fused_attr<double, 0, false>())) return rc;
+  if ((rc = set_fused_attr<double, 1, false>())) return rc;
+  void* fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+  if (qres != cudaDriverEntryPointSuccess || fn == nullptr) {
+    snprintf(g_state.cuda_msg, sizeof(g_state.cuda_msg), "cuTensorMapEncodeTiled not available from the driver");
+    return GAMER_HYDRO_CUDA_ERROR;
+  }
+  g_state.encode = reinterpret_cast<EncodeTiledFn>(fn);
+  g_state.device = device;
+  g_state.ready = true;
+  return 0;
+}
+
+int ensure_init() {
+  std::lock_guard<std::mutex> lk(g_mutex);
+  if (g_state.ready) return 0;
+  int dev = 0;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+  return init_locked(dev);
+}
+
+int ensure_scratch(size_t bytes) {
+  std::lock_guard<std::mutex> lk(g_mutex);
+  if (g_state.scratch_bytes >= bytes) return 0;
+  if (g_state.scratch) {
+    CK(cudaDeviceSynchronize());
+    CK(cudaFree(g_state.scratch));
+    g_state.scratch = nullptr;
+    g_state.scratch_bytes = 0;
+  }
+  CK(cudaMalloc(&g_state.scratch, bytes));
+  g_state.scratch_bytes = bytes;
+  return 0;
+}
+
+template <class R>
+size_t generic_scratch_bytes(int groups, int N, int ghost) {
+  const gh::GenericShape sh = gh::make_shape(N, ghost);
+  return (size_t)groups * (size_t)(sh.fs_stride + sh.fl_stride) * sizeof(R);
+}
+
+template <class R>
+int validate(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma, int limiter) {
+  if (n_groups < 0 || N < 1 || ghost < 2) return GAMER_HYDRO_INVALID_ARG;
+  if (!(dt > R(0)) || !(dx > R(0)) || !isfinite((double)dt) || !isfinite((double)dx)) return GAMER_HYDRO_INVALID_ARG;
+  if (!(gamma > R(1)) || !isfinite((double)gamma)) return GAMER_HYDRO_INVALID_ARG;
+  if (limiter != GAMER_HYDRO_MINMOD && limiter != GAMER_HYDRO_VANLEER) return GAMER_HYDRO_INVALID_ARG;
+  if (n_groups == 0) return 0;
+  if (!U_in || !U_out) return GAMER_HYDRO_INVALID_ARG;
+  if (((uintptr_t)U_in & 15) || ((uintptr_t)U_out & 15) || ((uintptr_t)bflux & 15)) return GAMER_HYDRO_INVALID_ARG;
+  return 0;
+}
+
+template <class R>
+bool fused_supported(int N, int ghost) {
+  // TMA: every global stride and the byte offset of the box start along x must be multiples of 16 bytes
+  // (measured on B200: a box starting at x = 1 float raises "illegal instruction").
+  const int S = N + 2 * ghost;
+  return N == gh::FN && ((S * (int)sizeof(R)) % 16 == 0) && (((ghost - 2) * (int)sizeof(R)) % 16 == 0);
+}
+
+template <class R>
+int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma, int limiter,
+                 cudaStream_t stream) {
+  const int S = N + 2 * ghost;
+  CUtensorMap map;
+  const cuuint64_t dims[5] = {(cuuint64_t)S, (cuuint64_t)S, (cuuint64_t)S, 5, (cuuint64_t)n_groups};
+  const cuuint64_t strides[4] = {(cuuint64_t)S * sizeof(R), (cuuint64_t)S * S * sizeof(R),
+                                 (cuuint64_t)S * S * S * sizeof(R), (cuuint64_t)5 * S * S * S * sizeof(R)};
+  const cuuint32_t box[5] = {(cuuint32_t)gh::FS, (cuuint32_t)gh::FS, 1, 5, 1};
+  const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
+  const CUtensorMapDataType dt_ = sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
+  CUresult r = g_state.encode(&map, dt_, 5, const_cast<R*>(U_in), dims, strides, box, estr,
+                              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    snprintf(g_state.cuda_msg, sizeof(g_state.cuda_msg), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
+    return GAMER_HYDRO_CUDA_ERROR;
+  }
+  const gh::GasConst<R> c = gh::make_consts<R>(dt, dx, gamma);
+  const int grid = n_groups < g_state.sm_count ? n_groups : g_state.sm_count;
+  const int smem = gh::FusedSmem<R>::total;
+  constexpr bool Fast = sizeof(R) == 4;
+  if (limiter == 0)
+    gh::fused_kernel<R, 0, Fast><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c,
+                                                                   g_state.status);
+  else
+    gh::fused_kernel<R, 1, Fast><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c,
+                                                                   g_state.status);
+  g_launches.fetch_add(1);
+  CK(cudaGetLastError());
+  return 0;
+}
+
+template <class R>
+int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma,
+                   int limiter, cudaStream_t stream) {
+  const int chunk = n_groups < kGenericChunk ? n_groups : kGenericChunk;
+  int rc = ensure_scratch(generic_scratch_bytes<R>(chunk, N, ghost));
+  if (rc) return rc;
+  const gh::GenericShape sh = gh::make_shape(N, ghost);
+  const gh::GasConst<R> c = gh::make_consts<R>(dt, dx, gamma);
+  R* FS = reinterpret_cast<R*>(g_state.scratch);
+  R* FL = FS + (size_t)chunk * sh.fs_stride;
+  const long long ne = (long long)sh.E * sh.E * sh.E, nf = 3LL * (N + 1) * N * N, nc = (long long)N * N * N;
+  for (int g0 = 0; g0 < n_groups; g0 += chunk) {
+    const int ng = (n_groups - g0) < chunk ? (n_groups - g0) : chunk;
+    const R* in = U_in + (size_t)g0 * sh.in_stride;
+    R* out = U_out + (size_t)g0 * sh.out_stride;
+    R* bf = bflux ? bflux + (size_t)g0 * 30 * N * N : nullptr;
+    const dim3 gp((unsigned)((ne + 127) / 128), ng), gf((unsigned)((nf + 127) / 128), ng),
+        gu((unsigned)((nc + 127) / 128), ng);
+    if (limiter == 0) gh::predict_kernel<R, 0><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status);
+    else gh::predict_kernel<R, 1><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status);
+    gh::flux_kernel<R><<<gf, 128, 0, stream>>>(FS, FL, bf, sh, c);
+    gh::update_kernel<R><<<gu, 128, 0, stream>>>(in, FL, out, sh, c, g_state.status);
+    g_launches.fetch_add(3);
+  }
+  CK(cudaGetLastError());
+  return 0;
+}
+
+template <class R>
+int step_impl(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma, int limiter,
+              cudaStream_t stream) {
+  int rc = validate<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter);
+  if (rc) return rc;
+  if (n_groups == 0) return 0;
+  if ((rc = ensure_init())) return rc;
+  int path = g_state.path;
+  if (path == GAMER_HYDRO_PATH_AUTO)
+    path = fused_supported<R>(N, ghost) ? GAMER_HYDRO_PATH_FUSED : GAMER_HYDRO_PATH_GENERIC;
+  if (path == GAMER_HYDRO_PATH_FUSED) {
+    if (!fused_supported<R>(N, ghost)) return GAMER_HYDRO_UNSUPPORTED;
+    return launch_fused<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+  }
+  return launch_generic<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+}
+
+void free_host_bufs() {
+  for (int s = 0; s < 3; ++s) {
+    if (g_state.hbuf_in[s]) cudaFree(g_state.hbuf_in[s]);
+    if (g_state.hbuf_out[s]) cudaFree(g_state.hbuf_out[s]);
+    if (g_state.hbuf_bf[s]) cudaFree(g_state.hbuf_bf[s]);
+    g_state.hbuf_in[s] = g_state.hbuf_out[s] = g_state.hbuf_bf[s] = nullptr;
+  }
+  g_state.hbuf_groups = 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gamer_hydro_alloc(int max_groups, int N, int ghost, int bytes_per_real, int device) {
+  if (max_groups < 0 || N < 1 || ghost < 2 || (bytes_per_real != 4 && bytes_per_real != 8))
+    return GAMER_HYDRO_INVALID_ARG;
+  {
+    std::lock_guard<std::mutex> lk(g_mutex);
+    int rc = init_locked(device);
+    if (rc) return rc;
+  }
+  const bool fused = bytes_per_real == 4 ? fused_supported<float>(N, ghost) : fused_supported<double>(N, ghost);
+  if (!fused && max_groups > 0) {
+    const int chunk = max_groups < kGenericChunk ? max_groups : kGenericChunk;
+    const size_t bytes = bytes_per_real == 4 ? generic_scratch_bytes<float>(chunk, N, ghost)
+                                             : generic_scratch_bytes<double>(chunk, N, ghost);
+    return ensure_scratch(bytes);
+  }
+  return 0;
+}
+
+void gamer_hydro_free(void) {
+  std::lock_guard<std::mutex> lk(g_mutex);
+  if (!g_state.ready) return;
+  cudaDeviceSynchronize();
+  free_host_bufs();
+  for (int s = 0; s < 3; ++s)
+    if (g_state.hstream[s]) { cudaStreamDestroy(g_state.hstream[s]); g_state.hstream[s] = nullptr; }
+  if (g_state.scratch) cudaFree(g_state.scratch);
+  if (g_state.status) cudaFree(g_state.status);
+  g_state.scratch = nullptr;
+  g_state.scratch_bytes = 0;
+  g_state.status = nullptr;
+  g_state.ready = false;
+  g_state.device = -1;
+}
+
+int gamer_hydro_step(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
+                     float gamma, int limiter, cudaStream_t stream) {
+  return step_impl<float>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+}
+
+int gamer_hydro_step_f64(const double* U_in, double* U_out, double* bflux, int n_groups, int N, int ghost, double dt,
+                         double dx, double gamma, int limiter, cudaStream_t stream) {
+  return step_impl<double>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+}
+
+int gamer_hydro_step_host(const float* h_in, float* h_out, float* h_bf, int n_groups, int N, int ghost, float dt,
+                          float dx, float gamma, int limiter, int chunk_groups) {
+  if (n_groups < 0 || N < 1 || ghost < 2) return GAMER_HYDRO_INVALID_ARG;
+  if (n_groups == 0) return 0;
+  if (!h_in || !h_out) return GAMER_HYDRO_INVALID_ARG;
+  int rc = ensure_init();
+  if (rc) return rc;
+  const size_t S = (size_t)N + 2 * ghost;
+  const size_t in_g = 5 * S * S * S, out_g = (size_t)5 * N * N * N, bf_g = (size_t)30 * N * N;
+  if (chunk_groups <= 0) chunk_groups = 1024;
+  if (chunk_groups > n_groups) chunk_groups = n_groups;
+  {
+    std::lock_guard<std::mutex> lk(g_mutex);
+    if (g_state.hbuf_groups < (size_t)chunk_groups || g_state.hbuf_N != N || g_state.hbuf_ghost != ghost) {
+      CK(cudaDeviceSynchronize());
+      free_host_bufs();
+      for (int s = 0; s < 3; ++s) {
+        if (!g_state.hstream[s]) CK(cudaStreamCreateWithFlags(&g_state.hstream[s], cudaStreamNonBlocking));
+        CK(cudaMalloc(&g_state.hbuf_in[s], chunk_groups * in_g * sizeof(float)));
+        CK(cudaMalloc(&g_state.hbuf_out[s], chunk_groups * out_g * sizeof(float)));
+        CK(cudaMalloc(&g_state.hbuf_bf[s], chunk_groups * bf_g * sizeof(float)));
+      }
+      g_state.hbuf_groups = chunk_groups;
+      g_state.hbuf_N = N;
+      g_state.hbuf_ghost = ghost;
+    }
+  }
+  int n = 0;
+  for (int g0 = 0; g0 < n_groups; g0 += chunk_groups, ++n) {
+    const int s = n % 3;
+    const int ng = (n_groups - g0) < chunk_groups ? (n_groups - g0) : chunk_groups;
+    cudaStream_t st = g_state.hstream[s];
+    float* d_in = (float*)g_state.hbuf_in[s];
+    float* d_out = (float*)g_state.hbuf_out[s];
+    float* d_bf = h_bf ? (float*)g_state.hbuf_bf[s] : nullptr;
+    CK(cudaMemcpyAsync(d_in, h_in + (size_t)g0 * in_g, ng * in_g * sizeof(float), cudaMemcpyHostToDevice, st));
+    rc = step_impl<float>(d_in, d_out, d_bf, ng, N, ghost, dt, dx, gamma, limiter, st);
+    if (rc) return rc;
+    CK(cudaMemcpyAsync(h_out + (size_t)g0 * out_g, d_out, ng * out_g * sizeof(float), cudaMemcpyDeviceToHost, st));
+    if (h_bf)
+      CK(cudaMemcpyAsync(h_bf + (size_t)g0 * bf_g, d_bf, ng * bf_g * sizeof(float), cudaMemcpyDeviceToHost, st));
+  }
+  for (int s = 0; s < 3; ++s) CK(cudaStreamSynchronize(g_state.hstream[s]));
+  return 0;
+}
+
+int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonpositive_out) {
+  int rc = ensure_init();
+  if (rc) return rc;
+  unsigned long long h[2];
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpy(h, g_state.status, sizeof(h), cudaMemcpyDeviceToHost));
+  CK(cudaMemset(g_state.status, 0, sizeof(h)));
+  if (guard_cells) *guard_cells = h[0];
+  if (nonpositive_out) *nonpositive_out = h[1];
+  return 0;
+}
+
+int gamer_hydro_set_path(int path) {
+  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED) return GAMER_HYDRO_INVALID_ARG;
+  g_state.path = path;
+  return 0;
+}
+
+unsigned long long gamer_hydro_launch_count(void) { return g_launches.load(); }
+
+const char* gamer_hydro_strerror(int code) {
+  switch (code) {
+    case GAMER_HYDRO_OK: return "success";
+    case GAMER_HYDRO_INVALID_ARG: return "invalid argument";
+    case GAMER_HYDRO_UNSUPPORTED: return "unsupported shape for the requested kernel path";
+    case GAMER_HYDRO_CUDA_ERROR: return g_state.cuda_msg;
+    case GAMER_HYDRO_NOT_SM100: return "device is not compute capability 10.x (sm_100a required)";
+    default: return "unknown error code";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,206 @@
+"""GPU parity tests proper (-m gpu): the CUDA path, called through the C ABI (via the thin binding), against
+the fp64 oracle element by element on identical seeded inputs. Tolerances are BASELINE.json:north_star's:
+fp32 <= 1e-4 max relative error (R14 metric) after one step, <= 1e-3 after 10 steps; fp64 <= 1e-11."""
+import numpy as np
+import pytest
+import torch
+
+import metrics
+import parity_util as pu
+import paper_1007_3818_b200 as gh
+from oracle import mhm_oracle as O
+from paper_1007_3818_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+G = wl.GAMMA
+TOL32_1, TOL32_10, TOL64 = 1e-4, 1e-3, 1e-11
+PATHS = [gh.PATH_FUSED, gh.PATH_GENERIC]
+
+
+def check(groups, dt, dx, limiter, path, tol, gamma=G, max_excl=pu.MAX_EXCLUDED_FRACTION, ghost=2):
+    out, bf, st = pu.run_gpu(groups, dt, dx, gamma, limiter, path=path, ghost=ghost)
+    assert np.isfinite(out).all() and np.isfinite(bf).all()
+    res = pu.compare(groups, dt, dx, gamma, limiter, out, bf, ghost=ghost)
+    assert res["excluded_fraction"] <= max_excl, res["excluded_fraction"]
+    assert res["err"] <= tol, res["err"]
+    assert res["err_bflux"] <= 10 * tol, res["err_bflux"]
+    return res, st
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg0_sod3d_one_step_fp32(path):
+    w = wl.config_0_sod3d()
+    res, st = check(w.groups(), w.dt(), pu.f32(w.dx), w.limiter, path, TOL32_1)
+    assert st == (res["oracle"].guard_cells, res["oracle"].nonpositive_out) == (0, 0)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg0_sod3d_one_step_fp64(path):
+    w = wl.config_0_sod3d()
+    check(w.groups(np.float64), w.dt(), w.dx, w.limiter, path, TOL64)
+
+
+@pytest.mark.parametrize("limiter", [0, 1])
+@pytest.mark.parametrize("path", PATHS)
+def test_random_states_fp32(path, limiter):
+    g = wl.random_groups(5, seed=101)
+    check(g, pu.f32(2e-3), pu.f32(1 / 16), limiter, path, TOL32_1)
+
+
+@pytest.mark.parametrize("limiter", [0, 1])
+@pytest.mark.parametrize("path", PATHS)
+def test_random_states_fp64(path, limiter):
+    g = wl.random_groups(3, seed=102, dtype=np.float64)
+    check(g, 2e-3, 1 / 16, limiter, path, TOL64)
+
+
+def test_many_groups_per_cta_and_ragged_tail():
+    """More groups than SMs and not a multiple of the grid: every CTA streams several groups through its TMA
+    ring and the last wave is ragged."""
+    n = 2 * 148 + 37
+    g = wl.random_groups(n, seed=103)
+    out, bf, st = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 0, path=gh.PATH_FUSED)
+    sample = np.r_[0:4, 146:152, 294:300, n - 3:n]
+    res = pu.compare(g[sample], pu.f32(2e-3), pu.f32(1 / 16), G, 0, out[sample], bf[sample])
+    assert res["err"] <= TOL32_1 and res["err_bflux"] <= 10 * TOL32_1
+    # deterministic and independent of the batch: any group run alone gives the same bits
+    out1, bf1, _ = pu.run_gpu(g[150:151], pu.f32(2e-3), pu.f32(1 / 16), G, 0, path=gh.PATH_FUSED)
+    assert np.array_equal(out1[0], out[150]) and np.array_equal(bf1[0], bf[150])
+    out2, _, _ = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 0, path=gh.PATH_FUSED)
+    assert np.array_equal(out2, out)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_uniform_moving_state_preserved_exactly(path):
+    W = (1.3, 0.37, -0.61, 0.23, 0.9)
+    U = wl.prim_box_to_cons(*(np.full((1, 1, 1), x) for x in W)).astype(np.float32).reshape(5)
+    g = np.broadcast_to(U[None, :, None, None, None], (3, 5, 20, 20, 20)).copy()
+    out, bf, st = pu.run_gpu(g, pu.f32(4e-3), pu.f32(1 / 32), G, 1, path=path)
+    assert np.array_equal(out, g[:, :, 2:-2, 2:-2, 2:-2])
+    assert st == (0, 0)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg2_turbulence_1_and_10_steps(path):
+    w = wl.config_2_turbulence(64, seed=2)
+    dx = pu.f32(w.dx)
+    res, st = check(w.groups(), w.dt(), dx, w.limiter, path, TOL32_1)
+    assert st[0] == 0
+    # 10 steps, GPU fp32 and oracle fp64 advanced independently from the same float32 start, same dt sequence
+    dts = []
+
+    def gpu_step(grp, dt):
+        dts.append(dt)
+        return pu.run_gpu(grp, dt, dx, G, w.limiter, path=path, want_bflux=False)[0]
+
+    Ug, t, _ = wl.advance(w.U, w.dx, w.bc, w.limiter, w.cfl, 10, gpu_step, dtype=np.float32)
+    Uo = w.U.astype(np.float64)
+    for dt in dts:
+        r = O.step_groups(wl.cut_groups(Uo, w.bc), 16, 2, dt, dx, G, w.limiter, want_bflux=False, want_guard=False)
+        Uo = wl.assemble_box(r.U_out, w.shape)
+    err = metrics.max_rel_err(Ug[None], Uo[None], G)
+    assert err <= TOL32_10, err
+    # conservation in the periodic box (P10), fp32 with fp64 accumulation
+    for q in range(5):
+        s0, s1 = w.U[q].astype(np.float64).sum(), Ug[q].astype(np.float64).sum()
+        assert abs(s1 - s0) <= 1e-5 * np.abs(w.U[q]).astype(np.float64).sum()
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_cfg3_cosmo_small_with_guard_accounting(path):
+    w = wl.config_3_cosmo(64, seed=3)
+    grp = w.groups()
+    res, st = check(grp, w.dt(), pu.f32(w.dx), w.limiter, path, TOL32_1, max_excl=1e-3)
+    o = res["oracle"]
+    assert o.guard_cells > 0
+    near = int((np.abs(o.margin) < pu.NEAR_GUARD).sum())
+    assert abs(st[0] - o.guard_cells) <= near, (st, o.guard_cells, near)
+
+
+def test_cfg1_sod_tube_steps_fp32_and_fp64():
+    w = wl.config_1_sod_tube(nx=256, steps=50)
+    for dtype, tol in ((np.float32, TOL32_10), (np.float64, 1e-9)):
+        dx = pu.f32(w.dx) if dtype == np.float32 else w.dx
+        dts = []
+
+        def gpu_step(grp, dt):
+            dts.append(dt)
+            return pu.run_gpu(grp, dt, dx, G, 0, want_bflux=False)[0]
+
+        Ug, t, _ = wl.advance(w.U.astype(dtype), w.dx, w.bc, 0, w.cfl, 10, gpu_step, dtype=dtype)
+        Uo = w.U.astype(np.float64)
+        for dt in dts:
+            r = O.step_groups(wl.cut_groups(Uo, w.bc), 16, 2, dt, dx, G, 0, want_bflux=False, want_guard=False)
+            Uo = wl.assemble_box(r.U_out, w.shape)
+        assert metrics.max_rel_err(Ug[None], Uo[None], G) <= tol
+        assert np.all(Ug[2] == 0) and np.all(Ug[3] == 0)     # transverse momentum stays exactly zero
+
+
+def test_generic_shapes_N8_ghost3_and_wider_ghost_shells():
+    g8 = wl.random_groups(4, seed=104, N=8, ghost=3)
+    out, bf, st = pu.run_gpu(g8, pu.f32(2e-3), pu.f32(1 / 8), G, 1, N=8, ghost=3)
+    r = O.step_groups(g8, 8, 3, pu.f32(2e-3), pu.f32(1 / 8), G, 1)
+    assert metrics.max_rel_err(out, r.U_out, G) <= TOL32_1
+    # wider shells: only the innermost two layers are read. ghost = 6 keeps the TMA box 16-byte aligned
+    # (fused path); ghost = 4 does not and is served by the generic path.
+    g = wl.random_groups(3, seed=105)
+    a = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 0, path=gh.PATH_FUSED)
+    for ghost, path in ((6, gh.PATH_FUSED), (4, gh.PATH_AUTO)):
+        gw = np.full((3, 5, 16 + 2 * ghost) + (16 + 2 * ghost,) * 2, np.nan, dtype=np.float32)
+        o = ghost - 2
+        gw[:, :, o:-o, o:-o, o:-o] = g
+        b = pu.run_gpu(gw, pu.f32(2e-3), pu.f32(1 / 16), G, 0, path=path, ghost=ghost)
+        if path == gh.PATH_FUSED:
+            assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+        else:
+            assert metrics.max_rel_err(b[0], a[0].astype(np.float64), G) <= 1e-5
+    with pytest.raises(gh.GamerHydroError):
+        pu.run_gpu(gw, pu.f32(2e-3), pu.f32(1 / 16), G, 0, path=gh.PATH_FUSED, ghost=4)
+
+
+def test_edge_cases_and_errors():
+    dev = torch.device("cuda", 0)
+    x = torch.zeros((0, 5, 20, 20, 20), device=dev)
+    out = torch.zeros((0, 5, 16, 16, 16), device=dev)
+    gh.gamer_hydro_step(x, out, None, 0, 16, 2, 1e-3, 1e-2, G, 0)            # empty batch is a no-op
+    x = torch.ones((1, 5, 20, 20, 20), device=dev)
+    out = torch.zeros((1, 5, 16, 16, 16), device=dev)
+    for kw in (dict(dt=0.0), dict(dt=float("nan")), dict(dx=-1.0), dict(gamma=1.0), dict(limiter=7)):
+        args = dict(dt=1e-3, dx=1e-2, gamma=G, limiter=0)
+        args.update(kw)
+        with pytest.raises(gh.GamerHydroError):
+            gh.gamer_hydro_step(x, out, None, 1, 16, 2, **args)
+    with pytest.raises(gh.GamerHydroError):      # ghost < 2
+        gh.gamer_hydro_step(torch.ones((1, 5, 18, 18, 18), device=dev), out, None, 1, 16, 1, 1e-3, 1e-2, G, 0)
+    # boundary_fluxes == NULL is allowed and does not change U_out
+    g = wl.random_groups(2, seed=106)
+    a = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 0, want_bflux=True)
+    b = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 0, want_bflux=False)
+    assert np.array_equal(a[0], b[0])
+    # garbage input (rho <= 0) neither hangs nor leaks into other groups
+    bad = g.copy()
+    bad[0, 0] = -1.0
+    c = pu.run_gpu(bad, pu.f32(2e-3), pu.f32(1 / 16), G, 0)
+    assert np.array_equal(c[0][1], a[0][1])
+
+
+def test_host_buffer_entry_point_matches_device_path():
+    g = wl.random_groups(50, seed=107)
+    dev_out, dev_bf, _ = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 1)
+    h_in = torch.from_numpy(g).pin_memory()
+    h_out = torch.empty((50, 5, 16, 16, 16), dtype=torch.float32).pin_memory()
+    h_bf = torch.empty((50, 6, 5, 16, 16), dtype=torch.float32).pin_memory()
+    gh.gamer_hydro_step_host(h_in, h_out, h_bf, 50, 16, 2, pu.f32(2e-3), pu.f32(1 / 16), G, 1, chunk_groups=16)
+    assert np.array_equal(h_out.numpy(), dev_out) and np.array_equal(h_bf.numpy(), dev_bf)
+
+
+def test_mirror_symmetry_gpu():
+    g = wl.random_groups(2, seed=108)
+    a = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 0)[0]
+    for axis in range(3):
+        m = np.flip(g, axis=4 - axis).copy()
+        m[:, 1 + axis] *= -1
+        b = pu.run_gpu(m, pu.f32(2e-3), pu.f32(1 / 16), G, 0)[0]
+        back = np.flip(b, axis=4 - axis).copy()
+        back[:, 1 + axis] *= -1
+        assert metrics.max_rel_err(back, a, G) <= 2e-6
