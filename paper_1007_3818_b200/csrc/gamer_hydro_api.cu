@@ -24,6 +24,7 @@ struct State {
   bool ready = false;
   int device = -1;
   int sm_count = 0;
+  int smem_per_sm = 0;
   unsigned long long* status = nullptr;  // [0] guard cells, [1] non-positive outputs
   void* scratch = nullptr;               // generic path: FS + FL for `scratch_groups` groups
   size_t scratch_bytes = 0;
@@ -73,6 +74,7 @@ int init_locked(int device) {
   if (prop.major != 10) return GAMER_HYDRO_NOT_SM100;
   CK(cudaSetDevice(device));
   g_state.sm_count = prop.multiProcessorCount;
+  g_state.smem_per_sm = (int)prop.sharedMemPerMultiprocessor;
   CK(cudaMalloc(&g_state.status, 2 * sizeof(unsigned long long)));
   CK(cudaMemset(g_state.status, 0, 2 * sizeof(unsigned long long)));
   int rc;
@@ -161,8 +163,11 @@ int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int gho
     return GAMER_HYDRO_CUDA_ERROR;
   }
   const gh::GasConst<R> c = gh::make_consts<R>(dt, dx, gamma);
-  const int grid = n_groups < g_state.sm_count ? n_groups : g_state.sm_count;
   const int smem = gh::FusedSmem<R>::total;
+  // persistent CTAs: as many as are resident at once (shared memory decides: 2 per SM in fp32, 1 in fp64)
+  const int per_sm = (2 * smem + 2048 <= g_state.smem_per_sm && gh::FMINB >= 2) ? 2 : 1;
+  const int resident = g_state.sm_count * per_sm;
+  const int grid = n_groups < resident ? n_groups : resident;
   constexpr bool Fast = sizeof(R) == 4;
   if (limiter == 0)
     gh::fused_kernel<R, 0, Fast><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c,

@@ -27,6 +27,10 @@ namespace gh {
 constexpr int FN = 16;              // interior cells per axis
 constexpr int FS = FN + 4;          // stored cells per axis that are read (2 ghost layers)
 constexpr int FNT = 320;            // threads per CTA
+#ifndef GH_FMINB
+#define GH_FMINB 2
+#endif
+constexpr int FMINB = GH_FMINB;     // resident CTAs per SM the kernel is compiled for
 constexpr int FPLANES = FN + 4;     // planes -2 .. 17 per group
 constexpr int FNSTAGE = 6;          // raw ring depth
 constexpr int WPITCH = 114;         // row pitch (reals) of the primitive plane: rows [r][q][c], 114 = 18 mod 32
@@ -78,7 +82,7 @@ __device__ __forceinline__ void tma_load_plane(uint32_t dst, const CUtensorMap* 
 }
 
 template <class R, int LIM, bool Fast>
-__global__ void __launch_bounds__(FNT, 1)
+__global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
     fused_kernel(const __grid_constant__ CUtensorMap in_map, R* __restrict__ U_out, R* __restrict__ bflux,
                  int n_groups, int goff, GasConst<R> c, unsigned long long* __restrict__ status) {
   using SM = FusedSmem<R>;
