@@ -45,8 +45,15 @@ enum {
 
 enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1 };
 
-/* kernel selection for gamer_hydro_set_path: AUTO picks FUSED when N == 16, else GENERIC */
-enum { GAMER_HYDRO_PATH_AUTO = 0, GAMER_HYDRO_PATH_GENERIC = 1, GAMER_HYDRO_PATH_FUSED = 2 };
+/* kernel selection for gamer_hydro_set_path: AUTO picks FUSED when N == 16, else GENERIC. FUSED is the
+ * performance path (fp32: two cells per thread, packed f32x2 arithmetic; fp64: one cell per thread);
+ * FUSED_SCALAR forces the one-cell-per-thread fused kernel in fp32 as well (a third implementation for tests). */
+enum {
+  GAMER_HYDRO_PATH_AUTO = 0,
+  GAMER_HYDRO_PATH_GENERIC = 1,
+  GAMER_HYDRO_PATH_FUSED = 2,
+  GAMER_HYDRO_PATH_FUSED_SCALAR = 3
+};
 
 /* One-time, idempotent, process-global set-up for `device`: checks the compute capability, raises the
  * dynamic shared-memory limits of the kernels, allocates the device status block and (for the generic

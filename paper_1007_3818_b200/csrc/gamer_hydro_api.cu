@@ -13,6 +13,7 @@
 #include "../../include/gamer_hydro.h"
 #include "hydro_fused.cuh"
 #include "hydro_generic.cuh"
+#include "hydro_pair.cuh"
 
 namespace {
 
@@ -82,6 +83,8 @@ int init_locked(int device) {
   if ((rc = set_fused_attr<float, 1, true>())) return rc;
   if ((rc = set_fused_attr<double, 0, false>())) return rc;
   if ((rc = set_fused_attr<double, 1, false>())) return rc;
+  CK(cudaFuncSetAttribute(gh::pair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
+  CK(cudaFuncSetAttribute(gh::pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
@@ -144,11 +147,10 @@ bool fused_supported(int N, int ghost) {
   return N == gh::FN && ((S * (int)sizeof(R)) % 16 == 0) && (((ghost - 2) * (int)sizeof(R)) % 16 == 0);
 }
 
+// rank-5 tensor map (x, y, z, var, group) over U_in; box = one z plane of all five variables (20 x 20 x 1 x 5 x 1)
 template <class R>
-int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma, int limiter,
-                 cudaStream_t stream) {
+int encode_plane_map(const R* U_in, int n_groups, int N, int ghost, CUtensorMap& map) {
   const int S = N + 2 * ghost;
-  CUtensorMap map;
   const cuuint64_t dims[5] = {(cuuint64_t)S, (cuuint64_t)S, (cuuint64_t)S, 5, (cuuint64_t)n_groups};
   const cuuint64_t strides[4] = {(cuuint64_t)S * sizeof(R), (cuuint64_t)S * S * sizeof(R),
                                  (cuuint64_t)S * S * S * sizeof(R), (cuuint64_t)5 * S * S * S * sizeof(R)};
@@ -162,6 +164,15 @@ int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int gho
     snprintf(g_state.cuda_msg, sizeof(g_state.cuda_msg), "cuTensorMapEncodeTiled failed with CUresult %d", (int)r);
     return GAMER_HYDRO_CUDA_ERROR;
   }
+  return 0;
+}
+
+template <class R>
+int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma, int limiter,
+                 cudaStream_t stream) {
+  CUtensorMap map;
+  int rc = encode_plane_map<R>(U_in, n_groups, N, ghost, map);
+  if (rc) return rc;
   const gh::GasConst<R> c = gh::make_consts<R>(dt, dx, gamma);
   const int smem = gh::FusedSmem<R>::total;
   // persistent CTAs: as many as are resident at once (shared memory decides: 2 per SM in fp32, 1 in fp64)
@@ -175,6 +186,26 @@ int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int gho
   else
     gh::fused_kernel<R, 1, Fast><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c,
                                                                    g_state.status);
+  g_launches.fetch_add(1);
+  CK(cudaGetLastError());
+  return 0;
+}
+
+// fp32 performance path: two cells per thread, packed f32x2 arithmetic (hydro_pair.cuh)
+int launch_pair(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
+                float gamma, int limiter, cudaStream_t stream) {
+  CUtensorMap map;
+  int rc = encode_plane_map<float>(U_in, n_groups, N, ghost, map);
+  if (rc) return rc;
+  const gh::PairConst c = gh::make_pair_consts(dt, dx, gamma);
+  const int smem = gh::PairSmem::total;
+  const int per_sm = (2 * (smem + 1024) <= g_state.smem_per_sm) ? 2 : 1;
+  const int resident = g_state.sm_count * per_sm;
+  const int grid = n_groups < resident ? n_groups : resident;
+  if (limiter == 0)
+    gh::pair_kernel<0><<<grid, gh::PNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  else
+    gh::pair_kernel<1><<<grid, gh::PNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   return 0;
@@ -218,8 +249,12 @@ int step_impl(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost,
   int path = g_state.path;
   if (path == GAMER_HYDRO_PATH_AUTO)
     path = fused_supported<R>(N, ghost) ? GAMER_HYDRO_PATH_FUSED : GAMER_HYDRO_PATH_GENERIC;
-  if (path == GAMER_HYDRO_PATH_FUSED) {
+  if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR) {
     if (!fused_supported<R>(N, ghost)) return GAMER_HYDRO_UNSUPPORTED;
+    if constexpr (sizeof(R) == 4) {
+      if (path == GAMER_HYDRO_PATH_FUSED)
+        return launch_pair(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+    }
     return launch_fused<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
   }
   return launch_generic<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
@@ -342,7 +377,7 @@ int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonp
 }
 
 int gamer_hydro_set_path(int path) {
-  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED) return GAMER_HYDRO_INVALID_ARG;
+  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_SCALAR) return GAMER_HYDRO_INVALID_ARG;
   g_state.path = path;
   return 0;
 }
