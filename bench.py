@@ -146,6 +146,8 @@ def main():
     ap.add_argument("--ref-groups", type=int, default=64)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused", "fused_scalar"],
+                    help="kernel path forced through gamer_hydro_set_path (default: the library's choice)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -171,6 +173,7 @@ def main():
     G = groups.shape[0]
     cells = G * N ** 3
     gh.gamer_hydro_alloc(G, N, GHOST, 4, local_rank)
+    gh.gamer_hydro_set_path({"auto": 0, "generic": 1, "fused": 2, "fused_scalar": 3}[args.path])
     h_in = torch.from_numpy(groups)
     d_in = h_in.to(dev)
     d_out = torch.empty((G, 5, N, N, N), dtype=torch.float32, device=dev)
@@ -301,7 +304,7 @@ def main():
                       "l2": "inputs (%.2f GB/step) far larger than the 126 MB L2; no flush needed" %
                             (h_in.numel() * 4 / 1e9),
                       "parallelism": "groups sharded across ranks, no collective",
-                      "generation_seconds": gen_s, "dt": dt, "dx": dx},
+                      "generation_seconds": gen_s, "dt": dt, "dx": dx, "kernel_path": args.path},
            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(launches),
            "clocks": clocks, "ms_per_step_min": min(per_step), "ms_per_step_median": float(np.median(per_step)),
            "guard_cells_per_step": guard_cells / args.steps, "nonpositive_out_per_step": nonpos / args.steps,

@@ -8,20 +8,21 @@
 //
 // Structure. N = 16. A CTA of 160 threads owns one patch group at a time and marches through
 // its z planes k = -1 .. 16. The 320 cells of a plane whose predicted face states are needed (18 x 18 cross:
-// interior + first ghost layer without the corners) are dealt out as 160 PAIRS (A, B) of cells of the same
-// column i, 9 rows apart (8 in the two ghost columns): both halves of every packed register run the same
-// instruction stream on two independent cells. Raw conserved planes arrive by TMA (5-D box loads) in a ring of
-// shared-memory stages, one mbarrier per stage. Per plane:
-//   A   cons -> prim of plane k+1 (own pair + the layer-2 / corner ghosts dealt to threads 0..33) -> primitive
-//       plane in shared memory (float4 + float per cell, double-buffered)
-//   B1  slopes, face values, own-direction face fluxes of plane k -> dU (half-step increment)
-//   B2  the six predicted face states as (rho, u, v, w, P, H); guard (reading R7); x+ / y+ states published;
-//       Roe flux at the lower z face (left state = previous plane's z+ state, kept in registers)
-//   -- barrier --
-//   D   Roe flux at the lower x and y faces; Fx, Fy published
-//   -- barrier --
-//   E   flux differences; conservative update of cell (i,j,k-1); U_out store; boundary-flux copy
-// Two CTAs are resident per SM so that one CTA's barrier wait is covered by the other.
+// interior + first ghost layer without the corners) are dealt out as 160 PAIRS of cells: warps 0..3 own the
+// 256 interior cells as x-adjacent pairs, warp 4 the 64 first-layer ghosts. Pairs are laid out in shared
+// memory so that own and y-neighbour accesses are single 64-bit loads / stores into packed registers. Raw
+// conserved planes arrive by TMA (5-D box loads) in a ring of shared-memory stages, one mbarrier per stage.
+// ONE CTA barrier per plane: everything a neighbour publishes is double-buffered and consumed one phase later.
+//   before the barrier of plane k:
+//     A   cons -> prim of plane k+1 (own pair; warp 4 also the layer-2 / corner ghosts) -> primitive plane
+//     B1  slopes, face values, own-direction face fluxes of plane k -> dU (half-step increment)
+//     B2  the six predicted face states as (rho, u, v, w, P, H); guard (reading R7); x+ / y+ states published;
+//         Roe flux at the lower z face (left state = previous plane's z+ state, kept in registers)
+//   after it:
+//     E   conservative update of cell (i,j,k-1) with the x / y fluxes of plane k-1 published one phase
+//         earlier; U_out store; boundary-flux copy
+//     D   Roe flux at the lower x and y faces of plane k; Fx, Fy published
+// Two CTAs are resident per SM (168 registers, 3 warps per sub-partition).
 #pragma once
 #include <cuda.h>
 #include <stdint.h>
@@ -245,7 +246,7 @@ __device__ __forceinline__ void roe2(const St2& L, const St2& R, const PairConst
   constexpr int t1 = (n + 1) % 3, t2 = (n + 2) % 3;
   const f2 Lv[3] = {L.u, L.v, L.w}, Rv[3] = {R.u, R.v, R.w};
   const f2 uL = Lv[n], vL = Lv[t1], wL = Lv[t2], uR = Rv[n], vR = Rv[t1], wR = Rv[t2];
-  const f2 z = sqrt2(R.r * rcp2(L.r));            // sqrt(rhoR / rhoL)
+  const f2 z = R.r * rsq2(L.r * R.r);             // sqrt(rhoR / rhoL) = rhoR / sqrt(rhoL rhoR)
   const f2 fR = z * rcp2(z + c.one);              // weight of the right state
   const f2 rt = L.r * z;                          // sqrt(rhoL rhoR)
   const f2 du = uR - uL, dv = vR - vL, dw = wR - wL, dH = R.h - L.h, dp = R.p - L.p, dr = R.r - L.r;
@@ -281,65 +282,60 @@ __device__ __forceinline__ void roe2(const St2& L, const St2& R, const PairConst
 }
 
 // ---- geometry of the pair kernel -----------------------------------------------------------------------------
+// 160 threads = 160 cell pairs (A, B) per plane = the 320 cells of the 18 x 18 cross whose predicted states are
+// needed. Pairs are chosen so that both cells of a pair, and both cells of each of its neighbour pairs in y, sit
+// in ADJACENT shared-memory slots: every own / y-neighbour access is one 64-bit LDS / STS straight into a packed
+// register pair.
+//   t <  128 : interior,   j = t / 8, A = (2p, j), B = (2p + 1, j), p = t % 8         (warps 0..3)
+//   t <  144 : row ghosts, j = -1 (t < 136) or 16, A = (2p, j), B = (2p + 1, j)        (warp 4, lanes 0..15)
+//   t <  160 : column ghosts, j = t - 144, A = (-1, j), B = (16, j)                    (warp 4, lanes 16..31)
+// All five warps run the same instruction stream; only per-thread offsets differ.
 constexpr int PNT = 160;          // threads per CTA = cell pairs per plane
 #ifndef GH_PREGS
-#define GH_PREGS 200
+#define GH_PREGS 168
 #endif
-constexpr int PREGS = GH_PREGS;   // registers per thread: 2 CTAs x 5 warps x 32 x 200 = 64000 of the 65536 per SM
-constexpr int PNSTAGE = 6;        // raw-plane ring depth
-constexpr int PHALF = 162;        // slots per half: 9 thread rows x 18 columns
-constexpr int PNSLOT = 392;       // 2 x 162 cross slots + 68 layer-2 / corner ghost slots
+constexpr int PREGS = GH_PREGS;   // 168 registers x 32 lanes x 3 warps fill one SM sub-partition's 16384 registers
+constexpr int PNSTAGE = 5;        // raw-plane ring depth
+constexpr int PNSLOT = 388;       // slots of a primitive plane (320 cross cells + 68 layer-2 / corner ghosts)
+constexpr int PNEX = 324;         // slots of an exchange array (interior + first ghost layer)
 constexpr int PRAW = 5 * FS * FS; // floats per raw plane (TMA box 20 x 20 x 1 x 5)
 
 struct PairSmem {
   static constexpr int raw_stage_bytes = ((PRAW * 4 + 127) / 128) * 128;
   static constexpr int raw_tx_bytes = PRAW * 4;
-  static constexpr int arr = PNSLOT * 4;                     // one quantity of one plane
   static constexpr int off_raw = 0;
-  static constexpr int off_w = off_raw + PNSTAGE * raw_stage_bytes;   // 2 primitive planes x 5
-  static constexpr int off_xs = off_w + 2 * 5 * arr;                  // x+ states, 6 quantities
-  static constexpr int off_ys = off_xs + 6 * arr;
-  static constexpr int off_fx = off_ys + 6 * arr;                     // Fx, 5 components
-  static constexpr int off_fy = off_fx + 5 * arr;
-  static constexpr int off_bar = ((off_fy + 5 * arr + 15) / 16) * 16;
+  static constexpr int off_w = off_raw + PNSTAGE * raw_stage_bytes;   // 2 buffers x 5 x PNSLOT primitives
+  static constexpr int off_xs = off_w + 2 * 5 * PNSLOT * 4;           // 2 x 6 x PNEX   x+ states
+  static constexpr int off_ys = off_xs + 2 * 6 * PNEX * 4;            // 2 x 6 x PNEX   y+ states
+  static constexpr int off_fx = off_ys + 2 * 6 * PNEX * 4;            // 2 x 5 x PNEX   Roe fluxes at lower x faces
+  static constexpr int off_fy = off_fx + 2 * 5 * PNEX * 4;            // 2 x 5 x PNEX   Roe fluxes at lower y faces
+  static constexpr int off_bar = ((off_fy + 2 * 5 * PNEX * 4 + 15) / 16) * 16;
   static constexpr int total = off_bar + PNSTAGE * 8 + 16;
 };
 
-// Slot of cell (i, j) of a plane in the shared-memory arrays. The 320 cross cells are laid out in THREAD order
-// (half, thread row, column) so that a warp's own-cell accesses are consecutive words; the 68 cells that are only
-// ever neighbours (layer-2 ghosts, inner corners) follow. Cells that are never read map to slot 0.
+// Slot of cell (i, j) of a plane. Interior cells row-major; ghost columns as [j][side] and ghost rows as
+// [side][i] so that the pairs named above are adjacent. Cells that are never read map to slot 0.
 __device__ __forceinline__ int pair_slot(int i, int j) {
   const bool in_x = (i >= 0 && i < FN), in_y = (j >= 0 && j < FN);
-  if (in_x && j >= -1 && j <= FN) return j <= 7 ? (j + 1) * 18 + (i + 1) : PHALF + (j - 8) * 18 + (i + 1);
-  if ((i == -1 || i == FN) && in_y) return j <= 7 ? (j + 1) * 18 + (i + 1) : PHALF + (j - 7) * 18 + (i + 1);
-  if (i == -2 && in_y) return 324 + j;
-  if (i == FN + 1 && in_y) return 340 + j;
-  if (j == -2 && in_x) return 356 + i;
-  if (j == FN + 1 && in_x) return 372 + i;
-  if (i == -1 && j == -1) return 388;
-  if (i == FN && j == -1) return 389;
-  if (i == -1 && j == FN) return 390;
-  if (i == FN && j == FN) return 391;
+  if (in_x && in_y) return FN * j + i;
+  if ((i == -1 || i == FN) && j >= -1 && j <= FN) return 256 + 2 * (j + 1) + (i == FN ? 1 : 0);
+  if ((j == -1 || j == FN) && in_x) return 292 + (j == FN ? FN : 0) + i;
+  if ((j == -2 || j == FN + 1) && in_x) return 324 + (j == FN + 1 ? FN : 0) + i;
+  if ((i == -2 || i == FN + 1) && in_y) return 356 + 2 * j + (i == FN + 1 ? 1 : 0);
   return 0;
 }
 
-__device__ __forceinline__ void st_state(float* base, int slot_a, int slot_b, const St2& s) {
-  const f2 q[6] = {s.r, s.u, s.v, s.w, s.p, s.h};
-#pragma unroll
-  for (int m = 0; m < 6; ++m) {
-    base[m * PNSLOT + slot_a] = lo(q[m]);
-    base[m * PNSLOT + slot_b] = hi(q[m]);
-  }
+__device__ __forceinline__ f2 lds2(const float* p) {   // one 64-bit shared load (p is 8-byte aligned)
+  f2 r;
+  r.v = *reinterpret_cast<const unsigned long long*>(p);
+  return r;
 }
-__device__ __forceinline__ St2 ld_state(const float* base, int slot_a, int slot_b) {
-  f2 q[6];
-#pragma unroll
-  for (int m = 0; m < 6; ++m) q[m] = mk2(base[m * PNSLOT + slot_a], base[m * PNSLOT + slot_b]);
-  St2 s;
-  s.r = q[0]; s.u = q[1]; s.v = q[2]; s.w = q[3]; s.p = q[4]; s.h = q[5];
-  return s;
-}
+__device__ __forceinline__ void sts2(float* p, f2 a) { *reinterpret_cast<unsigned long long*>(p) = a.v; }
 __device__ __forceinline__ f2 sel2(bool a, bool b, f2 x, f2 y) { return mk2(a ? lo(x) : lo(y), b ? hi(x) : hi(y)); }
+__device__ __forceinline__ void st_state2(float* base, int slot, const St2& s) {
+  sts2(base + 0 * PNEX + slot, s.r); sts2(base + 1 * PNEX + slot, s.u); sts2(base + 2 * PNEX + slot, s.v);
+  sts2(base + 3 * PNEX + slot, s.w); sts2(base + 4 * PNEX + slot, s.p); sts2(base + 5 * PNEX + slot, s.h);
+}
 
 template <int LIM>
 __global__ void __maxnreg__(PREGS)
@@ -355,32 +351,23 @@ __global__ void __maxnreg__(PREGS)
   const uint32_t raw_base = smem_u32(smem + SM::off_raw);
   const uint32_t bar_base = smem_u32(smem + SM::off_bar);
 
-  // ---- thread -> pair of cells (A, B): same column i, rows jA and jB
+  // ---- thread -> pair of cells (A, B)
   const int t = threadIdx.x;
-  int r, col;
-  if (t < 16) { r = 0; col = t + 1; }
-  else { r = 1 + (t - 16) / 18; col = (t - 16) % 18; }
-  const int i = col - 1;
-  const bool in_x = (i >= 0 && i < FN);
-  const int jA = r - 1, jB = in_x ? r + 8 : r + 7;
-  const bool inA = in_x && jA >= 0, inB = in_x && jB < FN;               // interior cells
-  const int oA = r * 18 + col, oB = oA + PHALF;                          // own slots
-  const int nxmA = pair_slot(i - 1, jA), nxpA = pair_slot(i + 1, jA);    // neighbour slots
-  const int nxmB = pair_slot(i - 1, jB), nxpB = pair_slot(i + 1, jB);
-  const int nymA = pair_slot(i, jA - 1), nypA = pair_slot(i, jA + 1);
-  const int nymB = pair_slot(i, jB - 1), nypB = pair_slot(i, jB + 1);
-  const int rawA = (jA + 2) * FS + (i + 2), rawB = (jB + 2) * FS + (i + 2);
-  const int outA = jA * FN + i, outB = jB * FN + i;
-  // the layer-2 / corner ghosts this thread converts as well (threads 0..33 only)
-  int eiA = 0, ejA = 0, eiB = 0, ejB = 0;
-  if (t < 16) { eiA = -2; ejA = t; eiB = FN + 1; ejB = t; }
-  else if (t < 32) { eiA = t - 16; ejA = -2; eiB = t - 16; ejB = FN + 1; }
-  else if (t == 32) { eiA = -1; ejA = -1; eiB = FN; ejB = -1; }
-  else if (t == 33) { eiA = -1; ejA = FN; eiB = FN; ejB = FN; }
-  const bool has_extra = t < 34;
-  const int rawEA = (ejA + 2) * FS + (eiA + 2), rawEB = (ejB + 2) * FS + (eiB + 2);
-  const int oEA = pair_slot(eiA, ejA), oEB = pair_slot(eiB, ejB);
-  // boundary-flux copy: thread -> (side, component, in-face index) of the x faces and of the y faces
+  const bool ghost_warp = t >= 128;  // warp-uniform: warp 4 owns the 64 first-layer ghost cells of a plane
+  int iA, jA, iB, jB;
+  if (t < 128) { jA = jB = t >> 3; iA = 2 * (t & 7); iB = iA + 1; }
+  else if (t < 144) { jA = jB = (t < 136) ? -1 : FN; iA = 2 * (t & 7); iB = iA + 1; }
+  else { jA = jB = t - 144; iA = -1; iB = FN; }
+  const int own = pair_slot(iA, jA);                                     // B sits in slot own + 1
+  const int xmA = pair_slot(iA - 1, jA), xmB = pair_slot(iB - 1, jB);    // x neighbours (scalar accesses)
+  const int xpA = pair_slot(iA + 1, jA), xpB = pair_slot(iB + 1, jB);
+  const int ym = pair_slot(iA, jA - 1), yp = pair_slot(iA, jA + 1);      // y neighbour pairs (64-bit accesses)
+  // the same neighbours inside the exchange arrays (PNEX slots); where the thread's face is never used the
+  // offset falls back to the thread's own slot, which always holds finite data
+  const int exA = xmA < PNEX ? xmA : own, exB = xmB < PNEX ? xmB : own + 1, eym = ym < PNEX ? ym : own;
+  const int rawA = (jA + 2) * FS + (iA + 2), rawB = (jB + 2) * FS + (iB + 2);
+  const int outo = jA * FN + iA;                                         // interior threads only
+  // boundary-flux copy: thread -> (side, component, in-face index) of the outer x faces and of the outer y faces
   const int bf_side = t / 80, bf_q = (t % 80) / 16, bf_m = t % 16;
   const int bfx_slot = pair_slot(bf_side ? FN : 0, bf_m), bfy_slot = pair_slot(bf_m, bf_side ? FN : 0);
 
@@ -411,25 +398,34 @@ __global__ void __maxnreg__(PREGS)
     return reinterpret_cast<const float*>(smem + SM::off_raw + (seq % PNSTAGE) * SM::raw_stage_bytes);
   };
   auto wait_plane = [&](int seq) { mbar_wait(bar_base + 8 * (seq % PNSTAGE), (seq / PNSTAGE) & 1); };
-  // cons -> prim of this thread's pair of plane `seq`; optionally published in the primitive plane
-  auto convert = [&](int seq, f2 W[5], bool publish, bool extras) {
-    const float* raw = raw_ptr(seq);
-    f2 U[5];
+  // conserved pair of a raw plane: one 64-bit load where the pair is adjacent in x (warps 0..3)
+  auto load_pair = [&](const float* raw, int a, int b, f2 U[5]) {
+    if (ghost_warp) {
 #pragma unroll
-    for (int q = 0; q < 5; ++q) U[q] = mk2(raw[q * (FS * FS) + rawA], raw[q * (FS * FS) + rawB]);
+      for (int q = 0; q < 5; ++q) U[q] = mk2(raw[q * (FS * FS) + a], raw[q * (FS * FS) + b]);
+    } else {
+#pragma unroll
+      for (int q = 0; q < 5; ++q) U[q] = lds2(raw + q * (FS * FS) + a);
+    }
+  };
+  auto publish_w = [&](float* wpl, int slot, const f2 W[5]) {
+#pragma unroll
+    for (int q = 0; q < 5; ++q) sts2(wpl + q * PNSLOT + slot, W[q]);
+  };
+  // warp 4 also converts the 68 cells of a plane that are only ever neighbours (layer-2 ghosts, inner corners)
+  auto convert_extras = [&](const float* raw, float* wpl) {
+    int a, b, slot;
+    if (t < 144) { const int jj = (t < 136) ? -2 : FN + 1; a = (jj + 2) * FS + (iA + 2); b = a + 1; slot = (t < 136) ? ym : yp; }
+    else { a = (jA + 2) * FS; b = a + FS - 1; slot = xmA; }
+    f2 U[5], W[5];
+    load_pair(raw, a, b, U);
     cons2prim2(U, c, W);
-    if (publish) {
-      float* wpl = wring + (seq & 1) * (5 * PNSLOT);
-#pragma unroll
-      for (int q = 0; q < 5; ++q) { wpl[q * PNSLOT + oA] = lo(W[q]); wpl[q * PNSLOT + oB] = hi(W[q]); }
-      if (extras && has_extra) {
-        f2 We[5];
-#pragma unroll
-        for (int q = 0; q < 5; ++q) U[q] = mk2(raw[q * (FS * FS) + rawEA], raw[q * (FS * FS) + rawEB]);
-        cons2prim2(U, c, We);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) { wpl[q * PNSLOT + oEA] = lo(We[q]); wpl[q * PNSLOT + oEB] = hi(We[q]); }
-      }
+    publish_w(wpl, slot, W);
+    if (t == 144 || t == 159) {  // inner corners (-1,-1),(16,-1) and (-1,16),(16,16)
+      const int jj = (t == 144) ? -1 : FN;
+      load_pair(raw, (jj + 2) * FS + 1, (jj + 2) * FS + FN + 2, U);
+      cons2prim2(U, c, W);
+      publish_w(wpl, t == 144 ? ym : yp, W);
     }
   };
 
@@ -437,170 +433,188 @@ __global__ void __maxnreg__(PREGS)
 
   for (int it = 0; it < n_local; ++it) {
     const int g = (int)blockIdx.x + it * (int)gridDim.x;
-    const int seq0 = it * FPLANES;  // sequence number of plane -2
+    const int seq0 = it * FPLANES;  // sequence number of plane -2 (even, so plane k lives in buffer k & 1)
     float* const outg = U_out + (size_t)g * (5 * FN * FN * FN);
     float* const bfg = bflux ? bflux + (size_t)g * (30 * FN * FN) : nullptr;
 
-    f2 Wm[5], Wc[5], Wp[5], acc[5], Fzm[5];
+    f2 Wc[5], dLz[5], accd[5], Fz[5];
     St2 zplus;
-    wait_plane(seq0);
-    convert(seq0, Wm, false, false);
-    wait_plane(seq0 + 1);
-    convert(seq0 + 1, Wc, true, false);
-    zplus.r = zplus.u = zplus.v = zplus.w = zplus.p = zplus.h = c.one;
+    {  // prologue: planes -2 and -1 of the thread's own pair
+      f2 U[5], Wm[5];
+      wait_plane(seq0);
+      load_pair(raw_ptr(seq0), rawA, rawB, U);
+      cons2prim2(U, c, Wm);
+      wait_plane(seq0 + 1);
+      load_pair(raw_ptr(seq0 + 1), rawA, rawB, U);
+      cons2prim2(U, c, Wc);
+      publish_w(wring + 5 * PNSLOT, own, Wc);
 #pragma unroll
-    for (int q = 0; q < 5; ++q) { acc[q] = c.one; Fzm[q] = c.one; }
+      for (int q = 0; q < 5; ++q) { dLz[q] = Wc[q] - Wm[q]; accd[q] = c.one; Fz[q] = c.one; }
+      zplus.r = zplus.u = zplus.v = zplus.w = zplus.p = zplus.h = c.one;
+    }
     __syncthreads();
+    if (t == 0) issue_upto(seq0 + 2 + PNSTAGE);
 
     for (int k = -1; k <= FN; ++k) {
       const int seq = seq0 + k + 2;  // sequence number of plane k
+      const int buf = k & 1;
       const bool ghost_plane = (k < 0 || k >= FN);
-      // ---- A: primitives of plane k+1
-      wait_plane(seq + 1);
-      convert(seq + 1, Wp, true, k + 1 < FN);
+      const bool active = !(ghost_warp && ghost_plane);  // warp-uniform: ghost cells of ghost planes are never used
 
-      // ---- B1: slopes, face values, own-direction fluxes -> dU
-      const float* wpl = wring + (seq & 1) * (5 * PNSLOT);
-      f2 sx[5], sy[5], sz[5], dU[5];
+      // ---- A: primitives of plane k+1 (own pair; warp 4 also the cells that are only neighbours)
+      f2 Wp[5];
       {
-        const f2 nrho = c.onen * Wc[0];
-        f2 dL[5], dR[5], accF[5];
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          dL[q] = Wc[q] - mk2(wpl[q * PNSLOT + nxmA], wpl[q * PNSLOT + nxmB]);
-          dR[q] = mk2(wpl[q * PNSLOT + nxpA], wpl[q * PNSLOT + nxpB]) - Wc[q];
-        }
-        predict_dir<0, LIM, true>(Wc, nrho, dL, dR, c, sx, accF);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          dL[q] = Wc[q] - mk2(wpl[q * PNSLOT + nymA], wpl[q * PNSLOT + nymB]);
-          dR[q] = mk2(wpl[q * PNSLOT + nypA], wpl[q * PNSLOT + nypB]) - Wc[q];
-        }
-        predict_dir<1, LIM, false>(Wc, nrho, dL, dR, c, sy, accF);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) { dL[q] = Wc[q] - Wm[q]; dR[q] = Wp[q] - Wc[q]; }
-        predict_dir<2, LIM, false>(Wc, nrho, dL, dR, c, sz, accF);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) dU[q] = c.hlamn * accF[q];
+        wait_plane(seq + 1);
+        const float* raw = raw_ptr(seq + 1);
+        f2 U[5];
+        load_pair(raw, rawA, rawB, U);
+        cons2prim2(U, c, Wp);
+        float* wpl = wring + (buf ^ 1) * (5 * PNSLOT);
+        if (k + 1 <= FN) publish_w(wpl, own, Wp);
+        if (ghost_warp && k + 1 >= 0 && k + 1 < FN) convert_extras(raw, wpl);
       }
+      f2 dRz[5];
+#pragma unroll
+      for (int q = 0; q < 5; ++q) dRz[q] = Wp[q] - Wc[q];
 
-      // ---- B2: the six predicted states; guard; publish x+ / y+; Roe at the lower z face
-      f2 gmin = c.one;
-      St2 xm = face_state<-1>(Wc, sx, dU, c, gmin);
-      St2 ym = face_state<-1>(Wc, sy, dU, c, gmin);
-      St2 zm = face_state<-1>(Wc, sz, dU, c, gmin);
-      St2 zp = face_state<+1>(Wc, sz, dU, c, gmin);
-      {
-        St2 xp = face_state<+1>(Wc, sx, dU, c, gmin);
-        St2 yp = face_state<+1>(Wc, sy, dU, c, gmin);
-        if (!ghost_plane) { st_state(xs, oA, oB, xp); st_state(ys, oA, oB, yp); }
-      }
-      {
-        // cells of the plane whose predicted states are used: the whole cross on interior planes, the interior on
-        // the two ghost planes. Only those may count as guard failures.
-        const bool useA = ghost_plane ? inA : true, useB = ghost_plane ? inB : true;
-        const bool okA = lo(gmin) > 0.0f, okB = hi(gmin) > 0.0f;
-        if (!(okA && okB)) {  // rare: first-order fallback for the failing cell(s) (reading R7)
-          St2 fb;
-          fb.r = Wc[0]; fb.u = Wc[1]; fb.v = Wc[2]; fb.w = Wc[3]; fb.p = Wc[4];
-          const f2 q = fma2(Wc[3], Wc[3], fma2(Wc[2], Wc[2], Wc[1] * Wc[1]));
-          fb.h = fma2(c.half, q, (c.gg1 * Wc[4]) * rcp2(Wc[0]));
-          auto fix = [&](St2& s) {
-            s.r = sel2(okA, okB, s.r, fb.r); s.u = sel2(okA, okB, s.u, fb.u); s.v = sel2(okA, okB, s.v, fb.v);
-            s.w = sel2(okA, okB, s.w, fb.w); s.p = sel2(okA, okB, s.p, fb.p); s.h = sel2(okA, okB, s.h, fb.h);
-          };
-          fix(xm); fix(ym); fix(zm); fix(zp);
-          if (!ghost_plane) {
-            const float fbv[6][2] = {{lo(fb.r), hi(fb.r)}, {lo(fb.u), hi(fb.u)}, {lo(fb.v), hi(fb.v)},
-                                     {lo(fb.w), hi(fb.w)}, {lo(fb.p), hi(fb.p)}, {lo(fb.h), hi(fb.h)}};
-#pragma unroll
-            for (int m = 0; m < 6; ++m) {
-              if (!okA) { xs[m * PNSLOT + oA] = fbv[m][0]; ys[m * PNSLOT + oA] = fbv[m][0]; }
-              if (!okB) { xs[m * PNSLOT + oB] = fbv[m][1]; ys[m * PNSLOT + oB] = fbv[m][1]; }
-            }
-          }
-          n_guard += ((!okA && useA) ? 1u : 0u) + ((!okB && useB) ? 1u : 0u);
-        }
-      }
-      f2 Fz[5];
-      if (k >= 0) {
-        roe2<2>(zplus, zm, c, Fz);
-        if (bfg && (k == 0 || k == FN)) {
-          float* p = bfg + (4 + (k == FN)) * (5 * FN * FN);
+      St2 xm, ymS;
+      if (active) {
+        // ---- B1: slopes, face values, own-direction fluxes -> dU
+        const float* wpl = wring + buf * (5 * PNSLOT);
+        f2 sx[5], sy[5], sz[5], dU[5];
+        {
+          const f2 nrho = c.onen * Wc[0];
+          f2 dL[5], dR[5], accF[5];
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            if (inA) p[q * (FN * FN) + outA] = lo(Fz[q]);
-            if (inB) p[q * (FN * FN) + outB] = hi(Fz[q]);
+            dL[q] = Wc[q] - mk2(wpl[q * PNSLOT + xmA], wpl[q * PNSLOT + xmB]);
+            dR[q] = mk2(wpl[q * PNSLOT + xpA], wpl[q * PNSLOT + xpB]) - Wc[q];
+          }
+          predict_dir<0, LIM, true>(Wc, nrho, dL, dR, c, sx, accF);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) {
+            dL[q] = Wc[q] - lds2(wpl + q * PNSLOT + ym);
+            dR[q] = lds2(wpl + q * PNSLOT + yp) - Wc[q];
+          }
+          predict_dir<1, LIM, false>(Wc, nrho, dL, dR, c, sy, accF);
+          predict_dir<2, LIM, false>(Wc, nrho, dLz, dRz, c, sz, accF);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) dU[q] = c.hlamn * accF[q];
+        }
+
+        // ---- B2: the six predicted states; guard; publish x+ / y+; Roe at the lower z face
+        f2 gmin = c.one;
+        {
+          const St2 xpS = face_state<+1>(Wc, sx, dU, c, gmin);
+          if (!ghost_plane) st_state2(xs + buf * (6 * PNEX), own, xpS);
+        }
+        {
+          const St2 ypS = face_state<+1>(Wc, sy, dU, c, gmin);
+          if (!ghost_plane) st_state2(ys + buf * (6 * PNEX), own, ypS);
+        }
+        xm = face_state<-1>(Wc, sx, dU, c, gmin);
+        ymS = face_state<-1>(Wc, sy, dU, c, gmin);
+        St2 zm = face_state<-1>(Wc, sz, dU, c, gmin);
+        St2 zp = face_state<+1>(Wc, sz, dU, c, gmin);
+        {
+          const bool okA = lo(gmin) > 0.0f, okB = hi(gmin) > 0.0f;
+          if (!(okA && okB)) {  // rare: first-order fallback for the failing cell(s) (reading R7)
+            St2 fb;
+            fb.r = Wc[0]; fb.u = Wc[1]; fb.v = Wc[2]; fb.w = Wc[3]; fb.p = Wc[4];
+            const f2 q = fma2(Wc[3], Wc[3], fma2(Wc[2], Wc[2], Wc[1] * Wc[1]));
+            fb.h = fma2(c.half, q, (c.gg1 * Wc[4]) * rcp2(Wc[0]));
+            auto fix = [&](St2& s) {
+              s.r = sel2(okA, okB, s.r, fb.r); s.u = sel2(okA, okB, s.u, fb.u); s.v = sel2(okA, okB, s.v, fb.v);
+              s.w = sel2(okA, okB, s.w, fb.w); s.p = sel2(okA, okB, s.p, fb.p); s.h = sel2(okA, okB, s.h, fb.h);
+            };
+            fix(xm); fix(ymS); fix(zm); fix(zp);
+            if (!ghost_plane) {
+              float* xsb = xs + buf * (6 * PNEX);
+              float* ysb = ys + buf * (6 * PNEX);
+              const float fbv[6][2] = {{lo(fb.r), hi(fb.r)}, {lo(fb.u), hi(fb.u)}, {lo(fb.v), hi(fb.v)},
+                                       {lo(fb.w), hi(fb.w)}, {lo(fb.p), hi(fb.p)}, {lo(fb.h), hi(fb.h)}};
+#pragma unroll
+              for (int m = 0; m < 6; ++m) {
+                if (!okA) { xsb[m * PNEX + own] = fbv[m][0]; ysb[m * PNEX + own] = fbv[m][0]; }
+                if (!okB) { xsb[m * PNEX + own + 1] = fbv[m][1]; ysb[m * PNEX + own + 1] = fbv[m][1]; }
+              }
+            }
+            n_guard += (okA ? 0u : 1u) + (okB ? 0u : 1u);   // every cell that gets here is one whose states are used
           }
         }
+        if (!ghost_warp && k >= 0) {
+          f2 Fn[5];
+          roe2<2>(zplus, zm, c, Fn);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) { accd[q] = Fn[q] - accd[q]; Fz[q] = Fn[q]; }  // upper z flux minus the lower-face sum
+          if (bfg && (k == 0 || k == FN)) {
+            float* p = bfg + (4 + (k == FN)) * (5 * FN * FN) + outo;
+#pragma unroll
+            for (int q = 0; q < 5; ++q) sts2(p + q * (FN * FN), Fn[q]);
+          }
+        }
+        zplus = zp;
       }
-      zplus = zp;
-      __syncthreads();  // S1: x+ / y+ states and primitive plane k+1 visible; raw planes <= k-2 retired
+      __syncthreads();  // x+ / y+ states of plane k, primitives of plane k+1, fluxes of plane k-1 visible
       if (t == 0) issue_upto(seq0 + k + 1 + PNSTAGE);
 
-      if (!ghost_plane) {
-        // ---- D: Roe fluxes at the lower x and y faces
-        f2 Fx[5], Fy[5];
-        {
-          const St2 L = ld_state(xs, nxmA, nxmB);
-          roe2<0>(L, xm, c, Fx);
-        }
-        {
-          const St2 L = ld_state(ys, nymA, nymB);
-          roe2<1>(L, ym, c, Fy);
-        }
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          fxs[q * PNSLOT + oA] = lo(Fx[q]); fxs[q * PNSLOT + oB] = hi(Fx[q]);
-          fys[q * PNSLOT + oA] = lo(Fy[q]); fys[q * PNSLOT + oB] = hi(Fy[q]);
-        }
-        __syncthreads();  // S2: Fx, Fy visible
-        // ---- E: finish cell (i,j,k-1) with its upper z flux, then start cell (i,j,k)
-        if (k >= 1) {
+      // ---- E: conservative update of plane k-1 (its x / y fluxes were published before this barrier)
+      if (k >= 1) {
+        const float* fxb = fxs + (buf ^ 1) * (5 * PNEX);
+        const float* fyb = fys + (buf ^ 1) * (5 * PNEX);
+        if (!ghost_warp) {
           const float* rawp = raw_ptr(seq - 1);
+          float* op = outg + (k - 1) * (FN * FN) + outo;
           f2 out[5];
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            const f2 Uin = mk2(rawp[q * (FS * FS) + rawA], rawp[q * (FS * FS) + rawB]);
-            out[q] = fma2(c.lamn, acc[q] + (Fz[q] - Fzm[q]), Uin);
-            if (inA) outg[(size_t)q * (FN * FN * FN) + (k - 1) * (FN * FN) + outA] = lo(out[q]);
-            if (inB) outg[(size_t)q * (FN * FN * FN) + (k - 1) * (FN * FN) + outB] = hi(out[q]);
+            const f2 Uin = lds2(rawp + q * (FS * FS) + rawA);
+            const f2 ux = mk2(fxb[q * PNEX + xpA], fxb[q * PNEX + xpB]);
+            const f2 uy = lds2(fyb + q * PNEX + yp);
+            out[q] = fma2(c.lamn, (ux + uy) + accd[q], Uin);
+            sts2(op + (size_t)q * (FN * FN * FN), out[q]);
           }
           const f2 m2 = fma2(out[3], out[3], fma2(out[2], out[2], out[1] * out[1]));
           const f2 tre = (out[0] + out[0]) * out[4];
-          n_nonpos += (inA && !(lo(out[0]) > 0.0f && lo(tre) > lo(m2)) ? 1u : 0u) +
-                      (inB && !(hi(out[0]) > 0.0f && hi(tre) > hi(m2)) ? 1u : 0u);
+          n_nonpos += (!(lo(out[0]) > 0.0f && lo(tre) > lo(m2)) ? 1u : 0u) +
+                      (!(hi(out[0]) > 0.0f && hi(tre) > hi(m2)) ? 1u : 0u);
+        }
+        if (bfg) {  // outer x and y faces of plane k-1: 2 sides x 5 components x 16 in-face cells each
+          bfg[((bf_side * 5 + bf_q) * FN + (k - 1)) * FN + bf_m] = fxb[bf_q * PNEX + bfx_slot];
+          bfg[(((2 + bf_side) * 5 + bf_q) * FN + (k - 1)) * FN + bf_m] = fyb[bf_q * PNEX + bfy_slot];
+        }
+      }
+      // ---- D: Roe fluxes at the lower x and y faces of plane k
+      if (!ghost_plane) {
+        const float* xsb = xs + buf * (6 * PNEX);
+        const float* ysb = ys + buf * (6 * PNEX);
+        float* fxo = fxs + buf * (5 * PNEX) + own;
+        float* fyo = fys + buf * (5 * PNEX) + own;
+        f2 Fx[5], Fy[5];
+        {
+          St2 L;
+          L.r = mk2(xsb[0 * PNEX + exA], xsb[0 * PNEX + exB]); L.u = mk2(xsb[1 * PNEX + exA], xsb[1 * PNEX + exB]);
+          L.v = mk2(xsb[2 * PNEX + exA], xsb[2 * PNEX + exB]); L.w = mk2(xsb[3 * PNEX + exA], xsb[3 * PNEX + exB]);
+          L.p = mk2(xsb[4 * PNEX + exA], xsb[4 * PNEX + exB]); L.h = mk2(xsb[5 * PNEX + exA], xsb[5 * PNEX + exB]);
+          roe2<0>(L, xm, c, Fx);
+        }
+#pragma unroll
+        for (int q = 0; q < 5; ++q) sts2(fxo + q * PNEX, Fx[q]);
+        {
+          St2 L;
+          L.r = lds2(ysb + 0 * PNEX + eym); L.u = lds2(ysb + 1 * PNEX + eym); L.v = lds2(ysb + 2 * PNEX + eym);
+          L.w = lds2(ysb + 3 * PNEX + eym); L.p = lds2(ysb + 4 * PNEX + eym); L.h = lds2(ysb + 5 * PNEX + eym);
+          roe2<1>(L, ymS, c, Fy);
         }
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          const f2 fxr = mk2(fxs[q * PNSLOT + nxpA], fxs[q * PNSLOT + nxpB]);
-          const f2 fyr = mk2(fys[q * PNSLOT + nypA], fys[q * PNSLOT + nypB]);
-          acc[q] = (fxr - Fx[q]) + (fyr - Fy[q]);
-          Fzm[q] = Fz[q];
+          sts2(fyo + q * PNEX, Fy[q]);
+          accd[q] = (Fx[q] + Fy[q]) + Fz[q];  // sum of the lower-face fluxes of plane k
         }
-        if (bfg) {  // outer x and y faces of this plane: 2 sides x 5 components x 16 in-face cells each
-          bfg[((bf_side * 5 + bf_q) * FN + k) * FN + bf_m] = fxs[bf_q * PNSLOT + bfx_slot];
-          bfg[(((2 + bf_side) * 5 + bf_q) * FN + k) * FN + bf_m] = fys[bf_q * PNSLOT + bfy_slot];
-        }
-      } else if (k == FN) {
-        const float* rawp = raw_ptr(seq - 1);
-        f2 out[5];
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          const f2 Uin = mk2(rawp[q * (FS * FS) + rawA], rawp[q * (FS * FS) + rawB]);
-          out[q] = fma2(c.lamn, acc[q] + (Fz[q] - Fzm[q]), Uin);
-          if (inA) outg[(size_t)q * (FN * FN * FN) + (k - 1) * (FN * FN) + outA] = lo(out[q]);
-          if (inB) outg[(size_t)q * (FN * FN * FN) + (k - 1) * (FN * FN) + outB] = hi(out[q]);
-        }
-        const f2 m2 = fma2(out[3], out[3], fma2(out[2], out[2], out[1] * out[1]));
-        const f2 tre = (out[0] + out[0]) * out[4];
-        n_nonpos += (inA && !(lo(out[0]) > 0.0f && lo(tre) > lo(m2)) ? 1u : 0u) +
-                    (inB && !(hi(out[0]) > 0.0f && hi(tre) > hi(m2)) ? 1u : 0u);
       }
 #pragma unroll
-      for (int q = 0; q < 5; ++q) { Wm[q] = Wc[q]; Wc[q] = Wp[q]; }
+      for (int q = 0; q < 5; ++q) { Wc[q] = Wp[q]; dLz[q] = dRz[q]; }
     }
-    __syncthreads();  // all reads of this group's planes and exchange arrays done before the next group starts
   }
 
   for (int o = 16; o > 0; o >>= 1) {
