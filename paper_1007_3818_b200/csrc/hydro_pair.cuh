@@ -310,7 +310,8 @@ struct PairSmem {
   static constexpr int off_fx = off_ys + 2 * 6 * PNEX * 4;            // 2 x 5 x PNEX   Roe fluxes at lower x faces
   static constexpr int off_fy = off_fx + 2 * 5 * PNEX * 4;            // 2 x 5 x PNEX   Roe fluxes at lower y faces
   static constexpr int off_bar = ((off_fy + 2 * 5 * PNEX * 4 + 15) / 16) * 16;
-  static constexpr int total = off_bar + PNSTAGE * 8 + 16;
+  static constexpr int off_sync = off_bar + PNSTAGE * 8;      // the CTA's split (arrive / wait) barrier
+  static constexpr int total = off_sync + 16;
 };
 
 // Slot of cell (i, j) of a plane. Interior cells row-major; ghost columns as [j][side] and ghost rows as
@@ -350,6 +351,7 @@ __global__ void __maxnreg__(PREGS)
   float* const fys = reinterpret_cast<float*>(smem + SM::off_fy);
   const uint32_t raw_base = smem_u32(smem + SM::off_raw);
   const uint32_t bar_base = smem_u32(smem + SM::off_bar);
+  const uint32_t sync_bar = smem_u32(smem + SM::off_sync);
 
   // ---- thread -> pair of cells (A, B)
   const int t = threadIdx.x;
@@ -359,17 +361,17 @@ __global__ void __maxnreg__(PREGS)
   else if (t < 144) { jA = jB = (t < 136) ? -1 : FN; iA = 2 * (t & 7); iB = iA + 1; }
   else { jA = jB = t - 144; iA = -1; iB = FN; }
   const int own = pair_slot(iA, jA);                                     // B sits in slot own + 1
-  const int xmA = pair_slot(iA - 1, jA), xmB = pair_slot(iB - 1, jB);    // x neighbours (scalar accesses)
-  const int xpA = pair_slot(iA + 1, jA), xpB = pair_slot(iB + 1, jB);
+  const int xmA = pair_slot(iA - 1, jA), xpB = pair_slot(iB + 1, jB);    // outer x neighbours (scalar accesses)
   const int ym = pair_slot(iA, jA - 1), yp = pair_slot(iA, jA + 1);      // y neighbour pairs (64-bit accesses)
-  // the same neighbours inside the exchange arrays (PNEX slots); where the thread's face is never used the
-  // offset falls back to the thread's own slot, which always holds finite data
-  const int exA = xmA < PNEX ? xmA : own, exB = xmB < PNEX ? xmB : own + 1, eym = ym < PNEX ? ym : own;
-  const int rawA = (jA + 2) * FS + (iA + 2), rawB = (jB + 2) * FS + (iB + 2);
-  const int outo = jA * FN + iA;                                         // interior threads only
-  // boundary-flux copy: thread -> (side, component, in-face index) of the outer x faces and of the outer y faces
-  const int bf_side = t / 80, bf_q = (t % 80) / 16, bf_m = t % 16;
-  const int bfx_slot = pair_slot(bf_side ? FN : 0, bf_m), bfy_slot = pair_slot(bf_m, bf_side ? FN : 0);
+  const int rawA = (jA + 2) * FS + (iA + 2);
+  // warp 4 only (recomputed where used so that they do not occupy registers in warps 0..3): the inner x
+  // neighbours of a column-ghost pair are not the pair's own cells, and its raw cells are not adjacent
+  auto xmB_of = [&]() { return pair_slot(iB - 1, jB); };
+  auto xpA_of = [&]() { return pair_slot(iA + 1, jA); };
+  auto rawB_of = [&]() { return (jB + 2) * FS + (iB + 2); };
+  // Neighbours inside the exchange arrays (PNEX slots): where the thread's face is never used the offset falls
+  // back to the thread's own slot, which always holds finite data.
+  const int exA = xmA < PNEX ? xmA : own;
 
   const int n_local = (n_groups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int total_planes = n_local * FPLANES;
@@ -388,11 +390,16 @@ __global__ void __maxnreg__(PREGS)
   };
   if (t == 0) {
     for (int s = 0; s < PNSTAGE; ++s) mbar_init(bar_base + 8 * s, 1);
+    mbar_init(sync_bar, PNT);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
   if (t == 0) issue_upto(PNSTAGE);
+  // split barrier: arrive once this plane's data is published, wait before reading the neighbours' data
+  uint32_t sync_phase = 0;
+  auto cta_arrive = [&]() { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(sync_bar) : "memory"); };
+  auto cta_wait = [&]() { mbar_wait(sync_bar, sync_phase); sync_phase ^= 1u; };
 
   auto raw_ptr = [&](int seq) -> const float* {
     return reinterpret_cast<const float*>(smem + SM::off_raw + (seq % PNSTAGE) * SM::raw_stage_bytes);
@@ -416,7 +423,7 @@ __global__ void __maxnreg__(PREGS)
   auto convert_extras = [&](const float* raw, float* wpl) {
     int a, b, slot;
     if (t < 144) { const int jj = (t < 136) ? -2 : FN + 1; a = (jj + 2) * FS + (iA + 2); b = a + 1; slot = (t < 136) ? ym : yp; }
-    else { a = (jA + 2) * FS; b = a + FS - 1; slot = xmA; }
+    else { a = (jA + 2) * FS; b = a + FS - 1; slot = xmA; }  // (-2, j) and (17, j)
     f2 U[5], W[5];
     load_pair(raw, a, b, U);
     cons2prim2(U, c, W);
@@ -442,10 +449,10 @@ __global__ void __maxnreg__(PREGS)
     {  // prologue: planes -2 and -1 of the thread's own pair
       f2 U[5], Wm[5];
       wait_plane(seq0);
-      load_pair(raw_ptr(seq0), rawA, rawB, U);
+      load_pair(raw_ptr(seq0), rawA, ghost_warp ? rawB_of() : 0, U);
       cons2prim2(U, c, Wm);
       wait_plane(seq0 + 1);
-      load_pair(raw_ptr(seq0 + 1), rawA, rawB, U);
+      load_pair(raw_ptr(seq0 + 1), rawA, ghost_warp ? rawB_of() : 0, U);
       cons2prim2(U, c, Wc);
       publish_w(wring + 5 * PNSLOT, own, Wc);
 #pragma unroll
@@ -467,7 +474,7 @@ __global__ void __maxnreg__(PREGS)
         wait_plane(seq + 1);
         const float* raw = raw_ptr(seq + 1);
         f2 U[5];
-        load_pair(raw, rawA, rawB, U);
+        load_pair(raw, rawA, ghost_warp ? rawB_of() : 0, U);
         cons2prim2(U, c, Wp);
         float* wpl = wring + (buf ^ 1) * (5 * PNSLOT);
         if (k + 1 <= FN) publish_w(wpl, own, Wp);
@@ -477,6 +484,9 @@ __global__ void __maxnreg__(PREGS)
 #pragma unroll
       for (int q = 0; q < 5; ++q) dRz[q] = Wp[q] - Wc[q];
 
+#pragma unroll
+      for (int q = 0; q < 5; ++q) { const f2 d = dRz[q]; dRz[q] = dLz[q]; dLz[q] = d; }  // dRz: lower, dLz: upper difference
+
       St2 xm, ymS;
       if (active) {
         // ---- B1: slopes, face values, own-direction fluxes -> dU
@@ -485,10 +495,19 @@ __global__ void __maxnreg__(PREGS)
         {
           const f2 nrho = c.onen * Wc[0];
           f2 dL[5], dR[5], accF[5];
+          if (ghost_warp) {
+            const int xmB = xmB_of(), xpA = xpA_of();
 #pragma unroll
-          for (int q = 0; q < 5; ++q) {
-            dL[q] = Wc[q] - mk2(wpl[q * PNSLOT + xmA], wpl[q * PNSLOT + xmB]);
-            dR[q] = mk2(wpl[q * PNSLOT + xpA], wpl[q * PNSLOT + xpB]) - Wc[q];
+            for (int q = 0; q < 5; ++q) {
+              dL[q] = Wc[q] - mk2(wpl[q * PNSLOT + xmA], wpl[q * PNSLOT + xmB]);
+              dR[q] = mk2(wpl[q * PNSLOT + xpA], wpl[q * PNSLOT + xpB]) - Wc[q];
+            }
+          } else {  // x-adjacent pair: the inner neighbours are the pair's own cells
+#pragma unroll
+            for (int q = 0; q < 5; ++q) {
+              dL[q] = Wc[q] - mk2(wpl[q * PNSLOT + xmA], lo(Wc[q]));
+              dR[q] = mk2(hi(Wc[q]), wpl[q * PNSLOT + xpB]) - Wc[q];
+            }
           }
           predict_dir<0, LIM, true>(Wc, nrho, dL, dR, c, sx, accF);
 #pragma unroll
@@ -497,7 +516,7 @@ __global__ void __maxnreg__(PREGS)
             dR[q] = lds2(wpl + q * PNSLOT + yp) - Wc[q];
           }
           predict_dir<1, LIM, false>(Wc, nrho, dL, dR, c, sy, accF);
-          predict_dir<2, LIM, false>(Wc, nrho, dLz, dRz, c, sz, accF);
+          predict_dir<2, LIM, false>(Wc, nrho, dRz, dLz, c, sz, accF);
 #pragma unroll
           for (int q = 0; q < 5; ++q) dU[q] = c.hlamn * accF[q];
         }
@@ -542,47 +561,46 @@ __global__ void __maxnreg__(PREGS)
             n_guard += (okA ? 0u : 1u) + (okB ? 0u : 1u);   // every cell that gets here is one whose states are used
           }
         }
+        // everything the neighbours need from this thread is published: arrive, then do the work that needs
+        // no neighbour (the z face) while the other warps catch up
+        cta_arrive();
         if (!ghost_warp && k >= 0) {
           f2 Fn[5];
           roe2<2>(zplus, zm, c, Fn);
 #pragma unroll
           for (int q = 0; q < 5; ++q) { accd[q] = Fn[q] - accd[q]; Fz[q] = Fn[q]; }  // upper z flux minus the lower-face sum
           if (bfg && (k == 0 || k == FN)) {
-            float* p = bfg + (4 + (k == FN)) * (5 * FN * FN) + outo;
+            float* p = bfg + (4 + (k == FN)) * (5 * FN * FN) + own;
 #pragma unroll
             for (int q = 0; q < 5; ++q) sts2(p + q * (FN * FN), Fn[q]);
           }
         }
         zplus = zp;
+      } else {
+        cta_arrive();
       }
-      __syncthreads();  // x+ / y+ states of plane k, primitives of plane k+1, fluxes of plane k-1 visible
+      cta_wait();  // x+ / y+ states of plane k, primitives of plane k+1, fluxes of plane k-1 visible
       if (t == 0) issue_upto(seq0 + k + 1 + PNSTAGE);
 
       // ---- E: conservative update of plane k-1 (its x / y fluxes were published before this barrier)
-      if (k >= 1) {
+      if (!ghost_warp && k >= 1) {
         const float* fxb = fxs + (buf ^ 1) * (5 * PNEX);
         const float* fyb = fys + (buf ^ 1) * (5 * PNEX);
-        if (!ghost_warp) {
-          const float* rawp = raw_ptr(seq - 1);
-          float* op = outg + (k - 1) * (FN * FN) + outo;
-          f2 out[5];
+        const float* rawp = raw_ptr(seq - 1);
+        float* op = outg + (k - 1) * (FN * FN) + own;
+        f2 out[5];
 #pragma unroll
-          for (int q = 0; q < 5; ++q) {
-            const f2 Uin = lds2(rawp + q * (FS * FS) + rawA);
-            const f2 ux = mk2(fxb[q * PNEX + xpA], fxb[q * PNEX + xpB]);
-            const f2 uy = lds2(fyb + q * PNEX + yp);
-            out[q] = fma2(c.lamn, (ux + uy) + accd[q], Uin);
-            sts2(op + (size_t)q * (FN * FN * FN), out[q]);
-          }
-          const f2 m2 = fma2(out[3], out[3], fma2(out[2], out[2], out[1] * out[1]));
-          const f2 tre = (out[0] + out[0]) * out[4];
-          n_nonpos += (!(lo(out[0]) > 0.0f && lo(tre) > lo(m2)) ? 1u : 0u) +
-                      (!(hi(out[0]) > 0.0f && hi(tre) > hi(m2)) ? 1u : 0u);
+        for (int q = 0; q < 5; ++q) {
+          const f2 Uin = lds2(rawp + q * (FS * FS) + rawA);
+          const f2 ux = mk2(fxb[q * PNEX + own + 1], fxb[q * PNEX + xpB]);
+          const f2 uy = lds2(fyb + q * PNEX + yp);
+          out[q] = fma2(c.lamn, (ux + uy) + accd[q], Uin);
+          sts2(op + (size_t)q * (FN * FN * FN), out[q]);
         }
-        if (bfg) {  // outer x and y faces of plane k-1: 2 sides x 5 components x 16 in-face cells each
-          bfg[((bf_side * 5 + bf_q) * FN + (k - 1)) * FN + bf_m] = fxb[bf_q * PNEX + bfx_slot];
-          bfg[(((2 + bf_side) * 5 + bf_q) * FN + (k - 1)) * FN + bf_m] = fyb[bf_q * PNEX + bfy_slot];
-        }
+        const f2 m2 = fma2(out[3], out[3], fma2(out[2], out[2], out[1] * out[1]));
+        const f2 tre = (out[0] + out[0]) * out[4];
+        n_nonpos += (!(lo(out[0]) > 0.0f && lo(tre) > lo(m2)) ? 1u : 0u) +
+                    (!(hi(out[0]) > 0.0f && hi(tre) > hi(m2)) ? 1u : 0u);
       }
       // ---- D: Roe fluxes at the lower x and y faces of plane k
       if (!ghost_plane) {
@@ -592,6 +610,7 @@ __global__ void __maxnreg__(PREGS)
         float* fyo = fys + buf * (5 * PNEX) + own;
         f2 Fx[5], Fy[5];
         {
+          const int exB = ghost_warp ? xmB_of() : own;
           St2 L;
           L.r = mk2(xsb[0 * PNEX + exA], xsb[0 * PNEX + exB]); L.u = mk2(xsb[1 * PNEX + exA], xsb[1 * PNEX + exB]);
           L.v = mk2(xsb[2 * PNEX + exA], xsb[2 * PNEX + exB]); L.w = mk2(xsb[3 * PNEX + exA], xsb[3 * PNEX + exB]);
@@ -601,6 +620,7 @@ __global__ void __maxnreg__(PREGS)
 #pragma unroll
         for (int q = 0; q < 5; ++q) sts2(fxo + q * PNEX, Fx[q]);
         {
+          const int eym = ym < PNEX ? ym : own;
           St2 L;
           L.r = lds2(ysb + 0 * PNEX + eym); L.u = lds2(ysb + 1 * PNEX + eym); L.v = lds2(ysb + 2 * PNEX + eym);
           L.w = lds2(ysb + 3 * PNEX + eym); L.p = lds2(ysb + 4 * PNEX + eym); L.h = lds2(ysb + 5 * PNEX + eym);
@@ -611,9 +631,33 @@ __global__ void __maxnreg__(PREGS)
           sts2(fyo + q * PNEX, Fy[q]);
           accd[q] = (Fx[q] + Fy[q]) + Fz[q];  // sum of the lower-face fluxes of plane k
         }
-      }
+        // ---- a5: the outer x and y faces of this plane (-x: cells i = 0; +x: column ghosts; -y: row 0; +y: row 16)
+        if (bfg) {
+          if (ghost_warp) {
+            if (t >= 144) {
 #pragma unroll
-      for (int q = 0; q < 5; ++q) { Wc[q] = Wp[q]; dLz[q] = dRz[q]; }
+              for (int q = 0; q < 5; ++q) bfg[((5 + q) * FN + k) * FN + jA] = hi(Fx[q]);
+            } else if (t >= 136) {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) sts2(bfg + ((15 + q) * FN + k) * FN + iA, Fy[q]);
+            }
+          } else {
+            if (iA == 0) {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) bfg[(q * FN + k) * FN + jA] = lo(Fx[q]);
+            }
+            if (t < 8) {
+#pragma unroll
+              for (int q = 0; q < 5; ++q) sts2(bfg + ((10 + q) * FN + k) * FN + iA, Fy[q]);
+            }
+          }
+        }
+      }
+      if (k < FN) {
+        const float* wnx = wring + (buf ^ 1) * (5 * PNSLOT) + own;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) Wc[q] = lds2(wnx + q * PNSLOT);
+      }
     }
   }
 
