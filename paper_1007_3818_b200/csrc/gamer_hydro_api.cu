@@ -395,4 +395,11 @@ const char* gamer_hydro_strerror(int code) {
   }
 }
 
+#ifdef GH_PROBE
+int gamer_hydro_probe(unsigned long long* out) {
+  cudaDeviceSynchronize();
+  return (int)cudaMemcpyFromSymbol(out, gh::gh_probe, sizeof(unsigned long long) * 80);
+}
+#endif
+
 }  // extern "C"

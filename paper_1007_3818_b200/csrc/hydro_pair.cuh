@@ -338,6 +338,10 @@ __device__ __forceinline__ void st_state2(float* base, int slot, const St2& s) {
   sts2(base + 3 * PNEX + slot, s.w); sts2(base + 4 * PNEX + slot, s.p); sts2(base + 5 * PNEX + slot, s.h);
 }
 
+#ifdef GH_PROBE
+__device__ unsigned long long gh_probe[4 * 5 * 4];
+#endif
+
 template <int LIM>
 __global__ void __maxnreg__(PREGS)
     pair_kernel(const __grid_constant__ CUtensorMap in_map, float* __restrict__ U_out, float* __restrict__ bflux,
@@ -371,21 +375,23 @@ __global__ void __maxnreg__(PREGS)
   auto rawB_of = [&]() { return (jB + 2) * FS + (iB + 2); };
   // Neighbours inside the exchange arrays (PNEX slots): where the thread's face is never used the offset falls
   // back to the thread's own slot, which always holds finite data.
-  const int exA = xmA < PNEX ? xmA : own;
+  const int exA = xmA < PNEX ? xmA : own;   // used by warps 0..3 only
 
   const int n_local = (n_groups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int total_planes = n_local * FPLANES;
-  int issued = 0;
-  auto issue_upto = [&](int limit) {  // thread 0 only
+  // TMA producer state (thread 0 only): next plane to request, kept incrementally (no div / mod on the hot path)
+  int issued = 0, iss_p = 0, iss_g = (int)blockIdx.x;
+  uint32_t iss_slot = 0;
+  auto issue_upto = [&](int limit) {
     if (limit > total_planes) limit = total_planes;
+#pragma unroll 1
     while (issued < limit) {
-      const int it = issued / FPLANES, p = issued % FPLANES;
-      const int slot = issued % PNSTAGE;
-      const int g = (int)blockIdx.x + it * (int)gridDim.x;
-      const uint32_t bar = bar_base + 8 * slot;
+      const uint32_t bar = bar_base + 8 * iss_slot;
       mbar_expect_tx(bar, SM::raw_tx_bytes);
-      tma_load_plane(raw_base + slot * SM::raw_stage_bytes, &in_map, goff, goff, goff + p, g, bar);
+      tma_load_plane(raw_base + iss_slot * SM::raw_stage_bytes, &in_map, goff, goff, goff + iss_p, iss_g, bar);
       ++issued;
+      if (++iss_p == FPLANES) { iss_p = 0; iss_g += (int)gridDim.x; }
+      if (++iss_slot == PNSTAGE) iss_slot = 0;
     }
   };
   if (t == 0) {
@@ -399,12 +405,21 @@ __global__ void __maxnreg__(PREGS)
   // split barrier: arrive once this plane's data is published, wait before reading the neighbours' data
   uint32_t sync_phase = 0;
   auto cta_arrive = [&]() { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(sync_bar) : "memory"); };
+#ifdef GH_PROBE
+  unsigned long long probe_wait = 0, probe_t0 = clock64(), probe_A = 0, probe_conv = 0, probe_ta = 0;
+  auto cta_wait = [&]() { const long long a = clock64(); mbar_wait(sync_bar, sync_phase); sync_phase ^= 1u; probe_wait += clock64() - a; };
+#else
   auto cta_wait = [&]() { mbar_wait(sync_bar, sync_phase); sync_phase ^= 1u; };
+#endif
 
-  auto raw_ptr = [&](int seq) -> const float* {
-    return reinterpret_cast<const float*>(smem + SM::off_raw + (seq % PNSTAGE) * SM::raw_stage_bytes);
+  // raw-ring consumer state: slot and mbarrier phase of the next plane this thread converts
+  uint32_t rs = 0, rph = 0;
+  auto next_plane = [&]() -> const float* {
+    mbar_wait(bar_base + 8 * rs, rph);
+    const float* p = reinterpret_cast<const float*>(smem + SM::off_raw + rs * SM::raw_stage_bytes);
+    if (++rs == PNSTAGE) { rs = 0; rph ^= 1u; }
+    return p;
   };
-  auto wait_plane = [&](int seq) { mbar_wait(bar_base + 8 * (seq % PNSTAGE), (seq / PNSTAGE) & 1); };
   // conserved pair of a raw plane: one 64-bit load where the pair is adjacent in x (warps 0..3)
   auto load_pair = [&](const float* raw, int a, int b, f2 U[5]) {
     if (ghost_warp) {
@@ -448,11 +463,9 @@ __global__ void __maxnreg__(PREGS)
     St2 zplus;
     {  // prologue: planes -2 and -1 of the thread's own pair
       f2 U[5], Wm[5];
-      wait_plane(seq0);
-      load_pair(raw_ptr(seq0), rawA, ghost_warp ? rawB_of() : 0, U);
+      load_pair(next_plane(), rawA, ghost_warp ? rawB_of() : 0, U);
       cons2prim2(U, c, Wm);
-      wait_plane(seq0 + 1);
-      load_pair(raw_ptr(seq0 + 1), rawA, ghost_warp ? rawB_of() : 0, U);
+      load_pair(next_plane(), rawA, ghost_warp ? rawB_of() : 0, U);
       cons2prim2(U, c, Wc);
       publish_w(wring + 5 * PNSLOT, own, Wc);
 #pragma unroll
@@ -463,16 +476,17 @@ __global__ void __maxnreg__(PREGS)
     if (t == 0) issue_upto(seq0 + 2 + PNSTAGE);
 
     for (int k = -1; k <= FN; ++k) {
-      const int seq = seq0 + k + 2;  // sequence number of plane k
       const int buf = k & 1;
       const bool ghost_plane = (k < 0 || k >= FN);
       const bool active = !(ghost_warp && ghost_plane);  // warp-uniform: ghost cells of ghost planes are never used
 
       // ---- A: primitives of plane k+1 (own pair; warp 4 also the cells that are only neighbours)
+#ifdef GH_PROBE
+      probe_ta = clock64();
+#endif
       f2 Wp[5];
       {
-        wait_plane(seq + 1);
-        const float* raw = raw_ptr(seq + 1);
+        const float* raw = next_plane();  // plane k+1
         f2 U[5];
         load_pair(raw, rawA, ghost_warp ? rawB_of() : 0, U);
         cons2prim2(U, c, Wp);
@@ -480,6 +494,9 @@ __global__ void __maxnreg__(PREGS)
         if (k + 1 <= FN) publish_w(wpl, own, Wp);
         if (ghost_warp && k + 1 >= 0 && k + 1 < FN) convert_extras(raw, wpl);
       }
+#ifdef GH_PROBE
+      probe_conv += clock64() - probe_ta;
+#endif
       f2 dRz[5];
 #pragma unroll
       for (int q = 0; q < 5; ++q) dRz[q] = Wp[q] - Wc[q];
@@ -522,6 +539,7 @@ __global__ void __maxnreg__(PREGS)
         }
 
         // ---- B2: the six predicted states; guard; publish x+ / y+; Roe at the lower z face
+        // ---- B2: the six predicted states; guard; publish x+ / y+
         f2 gmin = c.one;
         {
           const St2 xpS = face_state<+1>(Wc, sx, dU, c, gmin);
@@ -537,7 +555,7 @@ __global__ void __maxnreg__(PREGS)
         St2 zp = face_state<+1>(Wc, sz, dU, c, gmin);
         {
           const bool okA = lo(gmin) > 0.0f, okB = hi(gmin) > 0.0f;
-          if (!(okA && okB)) {  // rare: first-order fallback for the failing cell(s) (reading R7)
+          if (__builtin_expect(!(okA && okB), 0)) {  // rare: first-order fallback for the failing cell(s) (reading R7)
             St2 fb;
             fb.r = Wc[0]; fb.u = Wc[1]; fb.v = Wc[2]; fb.w = Wc[3]; fb.p = Wc[4];
             const f2 q = fma2(Wc[3], Wc[3], fma2(Wc[2], Wc[2], Wc[1] * Wc[1]));
@@ -563,6 +581,9 @@ __global__ void __maxnreg__(PREGS)
         }
         // everything the neighbours need from this thread is published: arrive, then do the work that needs
         // no neighbour (the z face) while the other warps catch up
+#ifdef GH_PROBE
+        probe_A += clock64() - probe_ta;
+#endif
         cta_arrive();
         if (!ghost_warp && k >= 0) {
           f2 Fn[5];
@@ -586,7 +607,8 @@ __global__ void __maxnreg__(PREGS)
       if (!ghost_warp && k >= 1) {
         const float* fxb = fxs + (buf ^ 1) * (5 * PNEX);
         const float* fyb = fys + (buf ^ 1) * (5 * PNEX);
-        const float* rawp = raw_ptr(seq - 1);
+        const int us = (int)rs - 3 + ((int)rs < 3 ? PNSTAGE : 0);  // slot of plane k-1 (rs points at plane k+2)
+        const float* rawp = reinterpret_cast<const float*>(smem + SM::off_raw + us * SM::raw_stage_bytes);
         float* op = outg + (k - 1) * (FN * FN) + own;
         f2 out[5];
 #pragma unroll
@@ -603,27 +625,25 @@ __global__ void __maxnreg__(PREGS)
                     (!(hi(out[0]) > 0.0f && hi(tre) > hi(m2)) ? 1u : 0u);
       }
       // ---- D: Roe fluxes at the lower x and y faces of plane k
-      if (!ghost_plane) {
+      if (!ghost_plane && !ghost_warp) {
         const float* xsb = xs + buf * (6 * PNEX);
         const float* ysb = ys + buf * (6 * PNEX);
         float* fxo = fxs + buf * (5 * PNEX) + own;
         float* fyo = fys + buf * (5 * PNEX) + own;
         f2 Fx[5], Fy[5];
-        {
-          const int exB = ghost_warp ? xmB_of() : own;
+        {  // faces (iA - 1/2) and (iA + 1/2): the second one lies between the pair's own cells
           St2 L;
-          L.r = mk2(xsb[0 * PNEX + exA], xsb[0 * PNEX + exB]); L.u = mk2(xsb[1 * PNEX + exA], xsb[1 * PNEX + exB]);
-          L.v = mk2(xsb[2 * PNEX + exA], xsb[2 * PNEX + exB]); L.w = mk2(xsb[3 * PNEX + exA], xsb[3 * PNEX + exB]);
-          L.p = mk2(xsb[4 * PNEX + exA], xsb[4 * PNEX + exB]); L.h = mk2(xsb[5 * PNEX + exA], xsb[5 * PNEX + exB]);
+          L.r = mk2(xsb[0 * PNEX + exA], xsb[0 * PNEX + own]); L.u = mk2(xsb[1 * PNEX + exA], xsb[1 * PNEX + own]);
+          L.v = mk2(xsb[2 * PNEX + exA], xsb[2 * PNEX + own]); L.w = mk2(xsb[3 * PNEX + exA], xsb[3 * PNEX + own]);
+          L.p = mk2(xsb[4 * PNEX + exA], xsb[4 * PNEX + own]); L.h = mk2(xsb[5 * PNEX + exA], xsb[5 * PNEX + own]);
           roe2<0>(L, xm, c, Fx);
         }
 #pragma unroll
         for (int q = 0; q < 5; ++q) sts2(fxo + q * PNEX, Fx[q]);
         {
-          const int eym = ym < PNEX ? ym : own;
           St2 L;
-          L.r = lds2(ysb + 0 * PNEX + eym); L.u = lds2(ysb + 1 * PNEX + eym); L.v = lds2(ysb + 2 * PNEX + eym);
-          L.w = lds2(ysb + 3 * PNEX + eym); L.p = lds2(ysb + 4 * PNEX + eym); L.h = lds2(ysb + 5 * PNEX + eym);
+          L.r = lds2(ysb + 0 * PNEX + ym); L.u = lds2(ysb + 1 * PNEX + ym); L.v = lds2(ysb + 2 * PNEX + ym);
+          L.w = lds2(ysb + 3 * PNEX + ym); L.p = lds2(ysb + 4 * PNEX + ym); L.h = lds2(ysb + 5 * PNEX + ym);
           roe2<1>(L, ymS, c, Fy);
         }
 #pragma unroll
@@ -631,25 +651,53 @@ __global__ void __maxnreg__(PREGS)
           sts2(fyo + q * PNEX, Fy[q]);
           accd[q] = (Fx[q] + Fy[q]) + Fz[q];  // sum of the lower-face fluxes of plane k
         }
-        // ---- a5: the outer x and y faces of this plane (-x: cells i = 0; +x: column ghosts; -y: row 0; +y: row 16)
+        // a5: outer faces -x (cells i = 0) and -y (row 0) of this plane
         if (bfg) {
-          if (ghost_warp) {
-            if (t >= 144) {
+          if (iA == 0) {
 #pragma unroll
-              for (int q = 0; q < 5; ++q) bfg[((5 + q) * FN + k) * FN + jA] = hi(Fx[q]);
-            } else if (t >= 136) {
+            for (int q = 0; q < 5; ++q) bfg[(q * FN + k) * FN + jA] = lo(Fx[q]);
+          }
+          if (t < 8) {
 #pragma unroll
-              for (int q = 0; q < 5; ++q) sts2(bfg + ((15 + q) * FN + k) * FN + iA, Fy[q]);
-            }
-          } else {
-            if (iA == 0) {
+            for (int q = 0; q < 5; ++q) sts2(bfg + ((10 + q) * FN + k) * FN + iA, Fy[q]);
+          }
+        }
+      } else if (!ghost_plane && t >= 136) {
+        // Warp 4: the only faces its cells own are x = 15.5 (B cells of the column ghosts) and y = 15.5 (row 16).
+        // One solve does both: the row-16 lanes rotate their states so that y is the normal direction.
+        const float* xsb = xs + buf * (6 * PNEX);
+        const float* ysb = ys + buf * (6 * PNEX);
+        const bool rowl = t < 144;
+        St2 L, R;
+        if (rowl) {
+          R.r = ymS.r; R.u = ymS.v; R.v = ymS.w; R.w = ymS.u; R.p = ymS.p; R.h = ymS.h;
+          L.r = lds2(ysb + 0 * PNEX + ym); L.u = lds2(ysb + 2 * PNEX + ym); L.v = lds2(ysb + 3 * PNEX + ym);
+          L.w = lds2(ysb + 1 * PNEX + ym); L.p = lds2(ysb + 4 * PNEX + ym); L.h = lds2(ysb + 5 * PNEX + ym);
+        } else {
+          const int exB = xmB_of();  // cell (15, j)
+          R = xm;
+          L.r = mk2(lo(xm.r), xsb[0 * PNEX + exB]); L.u = mk2(lo(xm.u), xsb[1 * PNEX + exB]);
+          L.v = mk2(lo(xm.v), xsb[2 * PNEX + exB]); L.w = mk2(lo(xm.w), xsb[3 * PNEX + exB]);
+          L.p = mk2(lo(xm.p), xsb[4 * PNEX + exB]); L.h = mk2(lo(xm.h), xsb[5 * PNEX + exB]);
+        }
+        f2 F[5];
+        roe2<0>(L, R, c, F);
+        if (rowl) {  // rotated back: normal -> my, first transverse -> mz, second -> mx
+          float* fyo = fys + buf * (5 * PNEX) + own;
+          sts2(fyo + 0 * PNEX, F[0]); sts2(fyo + 1 * PNEX, F[3]); sts2(fyo + 2 * PNEX, F[1]);
+          sts2(fyo + 3 * PNEX, F[2]); sts2(fyo + 4 * PNEX, F[4]);
+          if (bfg) {
+            float* p = bfg + (15 * FN + k) * FN + iA;
+            sts2(p + 0 * (FN * FN), F[0]); sts2(p + 1 * (FN * FN), F[3]); sts2(p + 2 * (FN * FN), F[1]);
+            sts2(p + 3 * (FN * FN), F[2]); sts2(p + 4 * (FN * FN), F[4]);
+          }
+        } else {
+          float* fxo = fxs + buf * (5 * PNEX) + own;
 #pragma unroll
-              for (int q = 0; q < 5; ++q) bfg[(q * FN + k) * FN + jA] = lo(Fx[q]);
-            }
-            if (t < 8) {
+          for (int q = 0; q < 5; ++q) sts2(fxo + q * PNEX, F[q]);
+          if (bfg) {
 #pragma unroll
-              for (int q = 0; q < 5; ++q) sts2(bfg + ((10 + q) * FN + k) * FN + iA, Fy[q]);
-            }
+            for (int q = 0; q < 5; ++q) bfg[((5 + q) * FN + k) * FN + jA] = hi(F[q]);
           }
         }
       }
@@ -661,6 +709,15 @@ __global__ void __maxnreg__(PREGS)
     }
   }
 
+#ifdef GH_PROBE
+  if ((t & 31) == 0 && blockIdx.x < 4) {
+    unsigned int wid, smid;
+    asm volatile("mov.u32 %0, %%warpid;" : "=r"(wid));
+    asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+    unsigned long long* pr = gh_probe + (blockIdx.x * 5 + (t >> 5)) * 4;
+    pr[0] = probe_wait; pr[1] = clock64() - probe_t0; pr[2] = probe_A; pr[3] = probe_conv;
+  }
+#endif
   for (int o = 16; o > 0; o >>= 1) {
     n_guard += __shfl_xor_sync(0xffffffffu, n_guard, o);
     n_nonpos += __shfl_xor_sync(0xffffffffu, n_nonpos, o);
