@@ -246,7 +246,7 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant (only) kernel: fused_kernel<float, MinMod>
+    # ---- roofline of the dominant (only) kernel of the step (pair_kernel<MinMod> on the default path)
     ms_launch = total_ms / args.steps                         # one launch per step on this rank
     flops = FLOPS_PER_CELL[w.limiter] * cells
     achieved_tf = flops / (ms_launch * 1e-3) / 1e12
@@ -262,7 +262,9 @@ def main():
         pass
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved_tf / ALU_PEAK_TFLOPS, "traffic": traffic,
-                "kernel": "gh::fused_kernel<float, MinMod>",
+                "kernel": {"auto": "gh::pair_kernel<MinMod>", "fused": "gh::pair_kernel<MinMod>",
+                           "fused_scalar": "gh::fused_kernel<float, MinMod, fast>",
+                           "generic": "gh::predict_kernel + flux_kernel + update_kernel"}[args.path],
                 "flops_per_cell_update": FLOPS_PER_CELL[w.limiter],
                 "peak_derivation": "148 SM x 128 FP32 lanes x 2 FLOP x 1.965 GHz (sm_max_mhz of MEASURED_PEAKS.json)",
                 "ms_per_launch": ms_launch,
