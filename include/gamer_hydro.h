@@ -52,7 +52,8 @@ enum {
   GAMER_HYDRO_PATH_AUTO = 0,
   GAMER_HYDRO_PATH_GENERIC = 1,
   GAMER_HYDRO_PATH_FUSED = 2,
-  GAMER_HYDRO_PATH_FUSED_SCALAR = 3
+  GAMER_HYDRO_PATH_FUSED_SCALAR = 3,
+  GAMER_HYDRO_PATH_FUSED_DUO = 4   /* fp32: one cell per thread, f32x2 lanes = two directions of the cell */
 };
 
 /* One-time, idempotent, process-global set-up for `device`: checks the compute capability, raises the

@@ -14,6 +14,7 @@
 #include "hydro_fused.cuh"
 #include "hydro_generic.cuh"
 #include "hydro_pair.cuh"
+#include "hydro_duo.cuh"
 
 namespace {
 
@@ -85,6 +86,8 @@ int init_locked(int device) {
   if ((rc = set_fused_attr<double, 1, false>())) return rc;
   CK(cudaFuncSetAttribute(gh::pair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
   CK(cudaFuncSetAttribute(gh::pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
+  CK(cudaFuncSetAttribute(gh::duo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DuoSmem::total));
+  CK(cudaFuncSetAttribute(gh::duo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DuoSmem::total));
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
@@ -191,6 +194,26 @@ int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int gho
   return 0;
 }
 
+// fp32, one cell per thread with the f32x2 lanes carrying two directions of the cell (hydro_duo.cuh)
+int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
+               float gamma, int limiter, cudaStream_t stream) {
+  CUtensorMap map;
+  int rc = encode_plane_map<float>(U_in, n_groups, N, ghost, map);
+  if (rc) return rc;
+  const gh::PairConst c = gh::make_pair_consts(dt, dx, gamma);
+  const int smem = gh::DuoSmem::total;
+  const int per_sm = (2 * (smem + 1024) <= g_state.smem_per_sm) ? 2 : 1;
+  const int resident = g_state.sm_count * per_sm;
+  const int grid = n_groups < resident ? n_groups : resident;
+  if (limiter == 0)
+    gh::duo_kernel<0><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  else
+    gh::duo_kernel<1><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  g_launches.fetch_add(1);
+  CK(cudaGetLastError());
+  return 0;
+}
+
 // fp32 performance path: two cells per thread, packed f32x2 arithmetic (hydro_pair.cuh)
 int launch_pair(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
                 float gamma, int limiter, cudaStream_t stream) {
@@ -249,11 +272,13 @@ int step_impl(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost,
   int path = g_state.path;
   if (path == GAMER_HYDRO_PATH_AUTO)
     path = fused_supported<R>(N, ghost) ? GAMER_HYDRO_PATH_FUSED : GAMER_HYDRO_PATH_GENERIC;
-  if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR) {
+  if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR || path == GAMER_HYDRO_PATH_FUSED_DUO) {
     if (!fused_supported<R>(N, ghost)) return GAMER_HYDRO_UNSUPPORTED;
     if constexpr (sizeof(R) == 4) {
       if (path == GAMER_HYDRO_PATH_FUSED)
         return launch_pair(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+      if (path == GAMER_HYDRO_PATH_FUSED_DUO)
+        return launch_duo(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
     }
     return launch_fused<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
   }
@@ -377,7 +402,7 @@ int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonp
 }
 
 int gamer_hydro_set_path(int path) {
-  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_SCALAR) return GAMER_HYDRO_INVALID_ARG;
+  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_DUO) return GAMER_HYDRO_INVALID_ARG;
   g_state.path = path;
   return 0;
 }

@@ -1,0 +1,402 @@
+// csrc/hydro_duo.cuh — fp32 performance path, variant "duo": ONE cell per thread (the 320-thread cross of
+// hydro_fused.cuh, 96 registers, two CTAs = 20 warps per SM) but with the two LANES of every Blackwell `*.f32x2`
+// instruction carrying two directions of the same cell instead of two cells:
+//   lanes (x, y)  for the '+' face states, the '-' face states, their own-direction fluxes and the x / y Roe solves
+//                 (the y lane holds its velocity components rotated (v, w, u) so that slot 1 is the normal one),
+//   lanes (z-, z+) for the two z face states and their fluxes.
+// The packed forms keep the issue-slot saving of hydro_pair.cuh (half the slots per FLOP) without its register
+// appetite, so five warps per scheduler stay resident to hide the dependent-issue latency (profiles/r1c_README.md).
+// Schedule per plane as in hydro_pair.cuh: ONE split (arrive / wait) CTA barrier, everything a neighbour publishes is
+// double-buffered and consumed one phase later. Follows PAPER.md:15 with the readings of DESIGN.md §3.
+#pragma once
+#include <cuda.h>
+#include <stdint.h>
+
+#include "hydro_pair.cuh"  // f2 helpers, PairConst, St2, roe2, limiters, mbarrier / TMA helpers
+
+namespace gh {
+
+constexpr int DNSTAGE = 5;   // raw-plane ring depth
+
+struct DuoSmem {
+  static constexpr int raw_stage_bytes = ((PRAW * 4 + 127) / 128) * 128;
+  static constexpr int raw_tx_bytes = PRAW * 4;
+  static constexpr int w_plane = WPITCH * FS;                       // floats per primitive plane, rows [r][q][c]
+  static constexpr int off_raw = 0;
+  static constexpr int off_w = off_raw + DNSTAGE * raw_stage_bytes;
+  static constexpr int off_xs = off_w + 2 * w_plane * 4;            // 2 x 6 x FNT  x+ states
+  static constexpr int off_ys = off_xs + 2 * 6 * FNT * 4;           // 2 x 6 x FNT  y+ states, velocities rotated
+  static constexpr int off_fx = off_ys + 2 * 6 * FNT * 4;           // 2 x 5 x FNT  Roe fluxes at lower x faces
+  static constexpr int off_fy = off_fx + 2 * 5 * FNT * 4;           // 2 x 5 x FNT  Roe fluxes at lower y faces (global order)
+  static constexpr int off_bar = ((off_fy + 2 * 5 * FNT * 4 + 15) / 16) * 16;
+  static constexpr int off_sync = off_bar + DNSTAGE * 8;
+  static constexpr int total = off_sync + 16;
+};
+
+// scalar state for the z-face solve
+struct St1 {
+  float r, u, v, w, p, h;
+};
+__device__ __forceinline__ St1 lane_lo(const St2& s) { return St1{lo(s.r), lo(s.u), lo(s.v), lo(s.w), lo(s.p), lo(s.h)}; }
+__device__ __forceinline__ St1 lane_hi(const St2& s) { return St1{hi(s.r), hi(s.u), hi(s.v), hi(s.w), hi(s.p), hi(s.h)}; }
+
+// own-direction physical flux of a packed face (step a2): slot N is the normal velocity of both lanes
+template <int N>
+__device__ __forceinline__ void flux_slot(const f2 W[5], const PairConst& c, f2 F[5]) {
+  const f2 mn = W[0] * W[N];
+  const f2 q = fma2(W[3], W[3], fma2(W[2], W[2], W[1] * W[1]));
+  const f2 e = fma2(c.half * W[0], q, c.gg1 * W[4]);      // E + P = gg1 P + 1/2 rho q
+  F[0] = mn;
+  F[1] = (N == 1) ? fma2(mn, W[1], W[4]) : mn * W[1];
+  F[2] = (N == 2) ? fma2(mn, W[2], W[4]) : mn * W[2];
+  F[3] = (N == 3) ? fma2(mn, W[3], W[4]) : mn * W[3];
+  F[4] = e * W[N];
+}
+
+// face values (primitives) + half-step increment -> predicted state (rho, velocities, P, H) of both lanes;
+// gmin accumulates min(rho, P) for the guard (reading R7)
+__device__ __forceinline__ St2 state_from_face(const f2 Wf[5], const f2 dU[5], const PairConst& c, f2& gmin) {
+  const f2 rb = Wf[0] + dU[0];
+  const f2 m1 = fma2(Wf[0], Wf[1], dU[1]), m2 = fma2(Wf[0], Wf[2], dU[2]), m3 = fma2(Wf[0], Wf[3], dU[3]);
+  const f2 q = fma2(Wf[3], Wf[3], fma2(Wf[2], Wf[2], Wf[1] * Wf[1]));
+  const f2 Eb = fma2(c.half * Wf[0], q, fma2(Wf[4], c.ig1, dU[4]));
+  const f2 r = rcp2(rb);
+  St2 o;
+  o.r = rb;
+  o.u = m1 * r;
+  o.v = m2 * r;
+  o.w = m3 * r;
+  const f2 ke2 = fma2(m3, o.w, fma2(m2, o.v, m1 * o.u));
+  o.p = fma2(c.hg1n, ke2, c.g1 * Eb);
+  o.h = (Eb + o.p) * r;
+  gmin = mk2(min3nan(lo(gmin), lo(rb), lo(o.p)), min3nan(hi(gmin), hi(rb), hi(o.p)));
+  return o;
+}
+
+// scalar Roe solve along z (same algebra as roe2<2>): flux density in global component order
+__device__ __forceinline__ void roe1_z(const St1& L, const St1& R, float g1, float F[5]) {
+  const float z = R.r * rsq1(L.r * R.r);
+  const float fR = z * rcp1(z + 1.0f);
+  const float rt = L.r * z;
+  const float du = R.w - L.w, dv = R.u - L.u, dw = R.v - L.v, dH = R.h - L.h, dp = R.p - L.p, dr = R.r - L.r;
+  const float u = fmaf(fR, du, L.w), v = fmaf(fR, dv, L.u), w = fmaf(fR, dw, L.v), H = fmaf(fR, dH, L.h);
+  const float q2 = fmaf(w, w, fmaf(v, v, u * u));
+  const float a2 = fmaf(-0.5f * g1, q2, g1 * H);
+  const float hq = 0.5f * q2;
+  const float rsa = rsq1(a2);
+  const float a = a2 * rsa;
+  const float t = dp * (rsa * rsa);
+  const float sg = (rt * du) * rsa;
+  const float l1 = u - a, l5 = u + a;
+  const float P4n = -0.25f * (fabsf(l5) + fabsf(l1)), M4n = -0.25f * (fabsf(l5) - fabsf(l1));
+  const float sN = fmaf(M4n, sg, P4n * t);
+  const float dN = fmaf(P4n, sg, M4n * t);
+  const float aun = -0.5f * fabsf(u);
+  const float c2N = (dr - t) * aun;
+  const float raN = rt * aun;
+  const float c3N = raN * dv, c4N = raN * dw;
+  const float D0 = sN + c2N;
+  const float ad = a * dN;
+  const float Dn = fmaf(u, D0, ad);
+  const float Dt1 = fmaf(v, D0, c3N), Dt2 = fmaf(w, D0, c4N);
+  const float D4 = fmaf(w, c4N, fmaf(v, c3N, fmaf(hq, c2N, fmaf(u, ad, H * sN))));
+  const float mL = L.r * L.w, mR = R.r * R.w;
+  F[0] = fmaf(0.5f, mL + mR, D0);
+  F[3] = fmaf(0.5f, fmaf(mL, L.w, L.p) + fmaf(mR, R.w, R.p), Dn);
+  F[1] = fmaf(0.5f, fmaf(mL, L.u, mR * R.u), Dt1);
+  F[2] = fmaf(0.5f, fmaf(mL, L.v, mR * R.v), Dt2);
+  F[4] = fmaf(0.5f, fmaf(mL, L.h, mR * R.h), D4);
+}
+
+template <int LIM>
+__device__ __forceinline__ float limited_slope1(float a, float b) {
+  if (LIM == 0) return minmod1(a, b);
+  const float p = a * b, s = a + b;
+  return vanleer1(a, b, p, s);
+}
+
+template <int LIM>
+__global__ void __launch_bounds__(FNT, 2)
+    duo_kernel(const __grid_constant__ CUtensorMap in_map, float* __restrict__ U_out, float* __restrict__ bflux,
+               int n_groups, int goff, const __grid_constant__ PairConst c, unsigned long long* __restrict__ status) {
+  using SM = DuoSmem;
+  extern __shared__ __align__(128) unsigned char smem[];
+  float* const wring = reinterpret_cast<float*>(smem + SM::off_w);
+  float* const xs = reinterpret_cast<float*>(smem + SM::off_xs);
+  float* const ys = reinterpret_cast<float*>(smem + SM::off_ys);
+  float* const fxs = reinterpret_cast<float*>(smem + SM::off_fx);
+  float* const fys = reinterpret_cast<float*>(smem + SM::off_fy);
+  const uint32_t raw_base = smem_u32(smem + SM::off_raw);
+  const uint32_t bar_base = smem_u32(smem + SM::off_bar);
+  const uint32_t sync_bar = smem_u32(smem + SM::off_sync);
+
+  // ---- thread -> cell (i, j) of the cross-shaped footprint (as in hydro_fused.cuh)
+  const int t = threadIdx.x;
+  int i, j;
+  if (t < 288) { j = t / 18; i = t % 18 - 1; }
+  else if (t < 304) { j = -1; i = t - 288; }
+  else { j = FN; i = t - 304; }
+  const bool in_x = (i >= 0 && i < FN), in_y = (j >= 0 && j < FN), interior = in_x && in_y;
+  auto tid_of = [](int ii, int jj) { return jj < 0 ? 288 + ii : (jj >= FN ? 304 + ii : jj * 18 + ii + 1); };
+  // the extra cell this thread also converts (layer-2 ghost behind a first-layer ghost; inner corners)
+  int ei = i, ej = j;
+  bool has_extra = true;
+  if (i == -1) ei = -2;
+  else if (i == FN) ei = FN + 1;
+  else if (j == -1) ej = -2;
+  else if (j == FN) ej = FN + 1;
+  else if ((i == 0 || i == FN - 1) && (j == 0 || j == FN - 1)) { ei = (i == 0) ? -1 : FN; ej = (j == 0) ? -1 : FN; }
+  else has_extra = false;
+  const int raw_own = (j + 2) * FS + (i + 2);            // [q][r][c] dense, + q*400
+  const int raw_ext = (ej + 2) * FS + (ei + 2);
+  const int w_own = (j + 2) * WPITCH + (i + 2);          // [r][q][c], + q*20
+  const int w_ext = (ej + 2) * WPITCH + (ei + 2);
+  const int t_xl = t > 0 ? t - 1 : 0;                    // thread (i-1, j): same row
+  const int t_xr = t + 1 < FNT ? t + 1 : t;              // thread (i+1, j)
+  const int t_yl = in_x ? tid_of(i, j - 1 < -1 ? -1 : j - 1) : t;   // thread (i, j-1)
+  const int t_yu = in_x ? tid_of(i, j + 1 > FN ? FN : j + 1) : t;   // thread (i, j+1)
+  const bool do_x = in_y && i >= 0;                      // owns the face (i-1/2, j), i in [0,16]
+  const bool do_y = in_x && j >= 0;                      // owns the face (i, j-1/2), j in [0,16]
+
+  const int n_local = (n_groups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int total_planes = n_local * FPLANES;
+  // TMA producer state (thread 0 only), kept incrementally
+  int issued = 0, iss_p = 0, iss_g = (int)blockIdx.x;
+  uint32_t iss_slot = 0;
+  auto issue_upto = [&](int limit) {
+    if (limit > total_planes) limit = total_planes;
+#pragma unroll 1
+    while (issued < limit) {
+      const uint32_t bar = bar_base + 8 * iss_slot;
+      mbar_expect_tx(bar, SM::raw_tx_bytes);
+      tma_load_plane(raw_base + iss_slot * SM::raw_stage_bytes, &in_map, goff, goff, goff + iss_p, iss_g, bar);
+      ++issued;
+      if (++iss_p == FPLANES) { iss_p = 0; iss_g += (int)gridDim.x; }
+      if (++iss_slot == DNSTAGE) iss_slot = 0;
+    }
+  };
+  if (t == 0) {
+    for (int s = 0; s < DNSTAGE; ++s) mbar_init(bar_base + 8 * s, 1);
+    mbar_init(sync_bar, FNT);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  }
+  __syncthreads();
+  if (t == 0) issue_upto(DNSTAGE);
+  uint32_t sync_phase = 0;
+  auto cta_arrive = [&]() { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(sync_bar) : "memory"); };
+  auto cta_wait = [&]() { mbar_wait(sync_bar, sync_phase); sync_phase ^= 1u; };
+  uint32_t rs = 0, rph = 0;  // raw-ring consumer state
+  auto next_plane = [&]() -> const float* {
+    mbar_wait(bar_base + 8 * rs, rph);
+    const float* p = reinterpret_cast<const float*>(smem + SM::off_raw + rs * SM::raw_stage_bytes);
+    if (++rs == DNSTAGE) { rs = 0; rph ^= 1u; }
+    return p;
+  };
+  const GasConst<float> gc = {lo(c.g1) + 1.0f, lo(c.g1), lo(c.ig1), lo(c.gg1), c.lam, 0.5f * c.lam};
+  auto convert = [&](const float* raw, int off, float W[5]) {
+    float U[5];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) U[q] = raw[q * (FS * FS) + off];
+    cons2prim<float, true>(U, gc, W);
+  };
+
+  unsigned int n_guard = 0, n_nonpos = 0;
+
+  for (int it = 0; it < n_local; ++it) {
+    const int g = (int)blockIdx.x + it * (int)gridDim.x;
+    const int seq0 = it * FPLANES;
+    float* const outg = U_out + (size_t)g * (5 * FN * FN * FN);
+    float* const bfg = bflux ? bflux + (size_t)g * (30 * FN * FN) : nullptr;
+
+    float Wc[5], dLz[5], accd[5], Fz[5];
+    St1 zplus;
+    {  // prologue: planes -2 and -1 of the thread's own cell
+      float Wm[5];
+      convert(next_plane(), raw_own, Wm);
+      convert(next_plane(), raw_own, Wc);
+      float* wpl = wring + SM::w_plane;  // plane -1 lives in buffer 1
+#pragma unroll
+      for (int q = 0; q < 5; ++q) { wpl[w_own + q * FS] = Wc[q]; dLz[q] = Wc[q] - Wm[q]; accd[q] = 1.0f; Fz[q] = 1.0f; }
+      zplus = St1{1.0f, 1.0f, 1.0f, 1.0f, 1.0f, 1.0f};
+    }
+    __syncthreads();
+    if (t == 0) issue_upto(seq0 + 2 + DNSTAGE);
+
+    for (int k = -1; k <= FN; ++k) {
+      const int buf = k & 1;
+      const bool ghost_plane = (k < 0 || k >= FN);
+      // ---- A: primitives of plane k+1 (own cell + the layer-2 / corner ghost this thread is responsible for)
+      float Wp[5], dRz[5];
+      {
+        const float* raw = next_plane();
+        convert(raw, raw_own, Wp);
+        float* wnext = wring + (buf ^ 1) * SM::w_plane;
+        if (k + 1 <= FN) {
+#pragma unroll
+          for (int q = 0; q < 5; ++q) wnext[w_own + q * FS] = Wp[q];
+        }
+        if (has_extra && k + 1 >= 0 && k + 1 < FN) {
+          float We[5];
+          convert(raw, raw_ext, We);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) wnext[w_ext + q * FS] = We[q];
+        }
+#pragma unroll
+        for (int q = 0; q < 5; ++q) dRz[q] = Wp[q] - Wc[q];
+      }
+
+      St2 SA;      // the x- and y- predicted states (lanes x, y)
+      St1 zm, zp;  // the z- and z+ predicted states
+      const bool do_pred = ghost_plane ? interior : true;
+      if (do_pred) {
+        // ---- B1: slopes, face values, own-direction fluxes -> dU
+        const float* wpl = wring + buf * SM::w_plane + w_own;
+        float sx[5], sy[5], sz[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          const float wc = Wc[q];
+          sx[q] = limited_slope1<LIM>(wc - wpl[q * FS - 1], wpl[q * FS + 1] - wc);
+          sy[q] = limited_slope1<LIM>(wc - wpl[q * FS - WPITCH], wpl[q * FS + WPITCH] - wc);
+          sz[q] = limited_slope1<LIM>(dLz[q], dRz[q]);
+        }
+        // lanes (x, y): the y lane carries (rho, v, w, u, P) so that slot 1 is the normal velocity of both lanes
+        const f2 sxy[5] = {mk2(sx[0], sy[0]), mk2(sx[1], sy[2]), mk2(sx[2], sy[3]), mk2(sx[3], sy[1]), mk2(sx[4], sy[4])};
+        const f2 Wrot[5] = {mk2(Wc[0], Wc[0]), mk2(Wc[1], Wc[2]), mk2(Wc[2], Wc[3]), mk2(Wc[3], Wc[1]), mk2(Wc[4], Wc[4])};
+        f2 WB[5], WA[5], WC[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          WB[q] = fma2(c.half, sxy[q], Wrot[q]);     // '+' faces
+          WA[q] = fma2(c.halfn, sxy[q], Wrot[q]);    // '-' faces
+          WC[q] = mk2(fmaf(-0.5f, sz[q], Wc[q]), fmaf(0.5f, sz[q], Wc[q]));  // lanes (z-, z+), not rotated
+        }
+        float d[5];
+        {
+          f2 FB[5], FA[5], FC[5], D[5];
+          flux_slot<1>(WB, c, FB);
+          flux_slot<1>(WA, c, FA);
+          flux_slot<3>(WC, c, FC);
+#pragma unroll
+          for (int q = 0; q < 5; ++q) D[q] = FB[q] - FA[q];
+          const float hl = lo(c.hlamn);
+          d[0] = hl * ((lo(D[0]) + hi(D[0])) + (hi(FC[0]) - lo(FC[0])));
+          d[1] = hl * ((lo(D[1]) + hi(D[3])) + (hi(FC[1]) - lo(FC[1])));
+          d[2] = hl * ((lo(D[2]) + hi(D[1])) + (hi(FC[2]) - lo(FC[2])));
+          d[3] = hl * ((lo(D[3]) + hi(D[2])) + (hi(FC[3]) - lo(FC[3])));
+          d[4] = hl * ((lo(D[4]) + hi(D[4])) + (hi(FC[4]) - lo(FC[4])));
+        }
+        const f2 dUrot[5] = {mk2(d[0], d[0]), mk2(d[1], d[2]), mk2(d[2], d[3]), mk2(d[3], d[1]), mk2(d[4], d[4])};
+        const f2 dUsp[5] = {mk2(d[0], d[0]), mk2(d[1], d[1]), mk2(d[2], d[2]), mk2(d[3], d[3]), mk2(d[4], d[4])};
+
+        // ---- B2: the six predicted states; guard; publish x+ / y+
+        f2 gmin = c.one;
+        {
+          const St2 SB = state_from_face(WB, dUrot, c, gmin);
+          if (!ghost_plane) {
+            float* xo = xs + buf * (6 * FNT) + t;
+            float* yo = ys + buf * (6 * FNT) + t;
+            xo[0 * FNT] = lo(SB.r); xo[1 * FNT] = lo(SB.u); xo[2 * FNT] = lo(SB.v);
+            xo[3 * FNT] = lo(SB.w); xo[4 * FNT] = lo(SB.p); xo[5 * FNT] = lo(SB.h);
+            yo[0 * FNT] = hi(SB.r); yo[1 * FNT] = hi(SB.u); yo[2 * FNT] = hi(SB.v);
+            yo[3 * FNT] = hi(SB.w); yo[4 * FNT] = hi(SB.p); yo[5 * FNT] = hi(SB.h);
+          }
+        }
+        SA = state_from_face(WA, dUrot, c, gmin);
+        St2 SC = state_from_face(WC, dUsp, c, gmin);
+        if (__builtin_expect(!(lo(gmin) > 0.0f && hi(gmin) > 0.0f), 0)) {
+          // rare: first-order fallback (reading R7) — all six states become the cell's own input state
+          const float q = fmaf(Wc[3], Wc[3], fmaf(Wc[2], Wc[2], Wc[1] * Wc[1]));
+          const float h = fmaf(0.5f, q, (lo(c.gg1) * Wc[4]) * rcp1(Wc[0]));
+          SA.r = mk2(Wc[0], Wc[0]); SA.u = mk2(Wc[1], Wc[2]); SA.v = mk2(Wc[2], Wc[3]); SA.w = mk2(Wc[3], Wc[1]);
+          SA.p = mk2(Wc[4], Wc[4]); SA.h = mk2(h, h);
+          SC.r = SA.r; SC.u = mk2(Wc[1], Wc[1]); SC.v = mk2(Wc[2], Wc[2]); SC.w = mk2(Wc[3], Wc[3]); SC.p = SA.p; SC.h = SA.h;
+          if (!ghost_plane) {
+            float* xo = xs + buf * (6 * FNT) + t;
+            float* yo = ys + buf * (6 * FNT) + t;
+            xo[0 * FNT] = Wc[0]; xo[1 * FNT] = Wc[1]; xo[2 * FNT] = Wc[2]; xo[3 * FNT] = Wc[3]; xo[4 * FNT] = Wc[4]; xo[5 * FNT] = h;
+            yo[0 * FNT] = Wc[0]; yo[1 * FNT] = Wc[2]; yo[2 * FNT] = Wc[3]; yo[3 * FNT] = Wc[1]; yo[4 * FNT] = Wc[4]; yo[5 * FNT] = h;
+          }
+          n_guard += 1u;  // every cell that gets here is one whose states are used
+        }
+        zm = lane_lo(SC);
+        zp = lane_hi(SC);
+      }
+      // everything the neighbours need from this thread is published: arrive, then the z face (needs no neighbour)
+      cta_arrive();
+      if (interior && k >= 0) {
+        float Fn[5];
+        roe1_z(zplus, zm, lo(c.g1), Fn);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { accd[q] = Fn[q] - accd[q]; Fz[q] = Fn[q]; }  // upper z flux minus the lower-face sum
+        if (bfg && (k == 0 || k == FN)) {
+          float* p = bfg + (4 + (k == FN)) * (5 * FN * FN) + j * FN + i;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) p[q * (FN * FN)] = Fn[q];
+        }
+      }
+      zplus = zp;
+      cta_wait();  // x+ / y+ states of plane k, primitives of plane k+1, fluxes of plane k-1 visible
+      if (t == 0) issue_upto(seq0 + k + 1 + DNSTAGE);
+
+      // ---- E: conservative update of plane k-1 (its x / y fluxes were published one phase earlier)
+      if (interior && k >= 1) {
+        const float* fxb = fxs + (buf ^ 1) * (5 * FNT) + t_xr;
+        const float* fyb = fys + (buf ^ 1) * (5 * FNT) + t_yu;
+        const int us = (int)rs - 3 + ((int)rs < 3 ? DNSTAGE : 0);  // slot of plane k-1 (rs points at plane k+2)
+        const float* rawp = reinterpret_cast<const float*>(smem + SM::off_raw + us * SM::raw_stage_bytes) + raw_own;
+        float* op = outg + (k - 1) * (FN * FN) + j * FN + i;
+        float out[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          out[q] = fmaf(-c.lam, (fxb[q * FNT] + fyb[q * FNT]) + accd[q], rawp[q * (FS * FS)]);
+          op[(size_t)q * (FN * FN * FN)] = out[q];
+        }
+        const float m2 = fmaf(out[3], out[3], fmaf(out[2], out[2], out[1] * out[1]));
+        n_nonpos += (out[0] > 0.0f && (out[0] + out[0]) * out[4] > m2) ? 0u : 1u;
+      }
+      // ---- D: Roe fluxes at the lower x face (lane x) and the lower y face (lane y) of plane k, one packed solve
+      if (!ghost_plane) {
+        const float* xl = xs + buf * (6 * FNT) + t_xl;
+        const float* yl = ys + buf * (6 * FNT) + t_yl;
+        St2 L;
+        L.r = mk2(xl[0 * FNT], yl[0 * FNT]); L.u = mk2(xl[1 * FNT], yl[1 * FNT]); L.v = mk2(xl[2 * FNT], yl[2 * FNT]);
+        L.w = mk2(xl[3 * FNT], yl[3 * FNT]); L.p = mk2(xl[4 * FNT], yl[4 * FNT]); L.h = mk2(xl[5 * FNT], yl[5 * FNT]);
+        f2 F[5];
+        roe2<0>(L, SA, c, F);
+        // lane x is in global component order; lane y comes back as (rho, my, mz, mx, E)
+        const float Fy[5] = {hi(F[0]), hi(F[3]), hi(F[1]), hi(F[2]), hi(F[4])};
+        float* fxo = fxs + buf * (5 * FNT) + t;
+        float* fyo = fys + buf * (5 * FNT) + t;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) {
+          fxo[q * FNT] = lo(F[q]);
+          fyo[q * FNT] = Fy[q];
+          accd[q] = (lo(F[q]) + Fy[q]) + Fz[q];  // sum of the lower-face fluxes of plane k
+        }
+        if (bfg) {  // a5: outer faces of this plane
+          if (do_x && (i == 0 || i == FN)) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) bfg[(((i == FN ? 5 : 0) + q) * FN + k) * FN + j] = lo(F[q]);
+          }
+          if (do_y && (j == 0 || j == FN)) {
+#pragma unroll
+            for (int q = 0; q < 5; ++q) bfg[(((j == FN ? 15 : 10) + q) * FN + k) * FN + i] = Fy[q];
+          }
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < 5; ++q) { Wc[q] = Wp[q]; dLz[q] = dRz[q]; }
+    }
+  }
+
+  for (int o = 16; o > 0; o >>= 1) {
+    n_guard += __shfl_xor_sync(0xffffffffu, n_guard, o);
+    n_nonpos += __shfl_xor_sync(0xffffffffu, n_nonpos, o);
+  }
+  if ((t & 31) == 0) {
+    if (n_guard) atomicAdd(&status[0], (unsigned long long)n_guard);
+    if (n_nonpos) atomicAdd(&status[1], (unsigned long long)n_nonpos);
+  }
+}
+
+}  // namespace gh
