@@ -2,8 +2,8 @@
 // hydro_fused.cuh, 96 registers, two CTAs = 20 warps per SM) but with the two LANES of every Blackwell `*.f32x2`
 // instruction carrying two directions of the same cell instead of two cells:
 //   lanes (x, y)  for the '+' face states, the '-' face states, their own-direction fluxes and the x / y Roe solves
-//                 (the y lane holds its velocity components rotated (v, w, u) so that slot 1 is the normal one),
-//   lanes (z-, z+) for the two z face states and their fluxes.
+//                 (the y lane holds its velocity components as (v, u, w) so that slot 1 is the normal one),
+//   lanes (z-, z+) for the two z face states and their fluxes (same slot orders, slot 3 = w is normal in both).
 // The packed forms keep the issue-slot saving of hydro_pair.cuh (half the slots per FLOP) without its register
 // appetite, so five warps per scheduler stay resident to hide the dependent-issue latency (profiles/r1c_README.md).
 // Schedule per plane as in hydro_pair.cuh: ONE split (arrive / wait) CTA barrier, everything a neighbour publishes is
@@ -24,11 +24,9 @@ struct DuoSmem {
   static constexpr int w_plane = WPITCH * FS;                       // floats per primitive plane, rows [r][q][c]
   static constexpr int off_raw = 0;
   static constexpr int off_w = off_raw + DNSTAGE * raw_stage_bytes;
-  static constexpr int off_xs = off_w + 2 * w_plane * 4;            // 2 x 6 x FNT  x+ states
-  static constexpr int off_ys = off_xs + 2 * 6 * FNT * 4;           // 2 x 6 x FNT  y+ states, velocities rotated
-  static constexpr int off_fx = off_ys + 2 * 6 * FNT * 4;           // 2 x 5 x FNT  Roe fluxes at lower x faces
-  static constexpr int off_fy = off_fx + 2 * 5 * FNT * 4;           // 2 x 5 x FNT  Roe fluxes at lower y faces (global order)
-  static constexpr int off_bar = ((off_fy + 2 * 5 * FNT * 4 + 15) / 16) * 16;
+  static constexpr int off_st = off_w + 2 * w_plane * 4;            // 2 x 6 x FNT x (x+ state, y+ state in slot order)
+  static constexpr int off_fl = off_st + 2 * 6 * FNT * 8;           // 2 x 5 x FNT x (Fx, Fy in slot order) at the lower faces
+  static constexpr int off_bar = ((off_fl + 2 * 5 * FNT * 8 + 15) / 16) * 16;
   static constexpr int off_sync = off_bar + DNSTAGE * 8;
   static constexpr int total = off_sync + 16;
 };
@@ -122,10 +120,8 @@ __global__ void __launch_bounds__(FNT, 2)
   using SM = DuoSmem;
   extern __shared__ __align__(128) unsigned char smem[];
   float* const wring = reinterpret_cast<float*>(smem + SM::off_w);
-  float* const xs = reinterpret_cast<float*>(smem + SM::off_xs);
-  float* const ys = reinterpret_cast<float*>(smem + SM::off_ys);
-  float* const fxs = reinterpret_cast<float*>(smem + SM::off_fx);
-  float* const fys = reinterpret_cast<float*>(smem + SM::off_fy);
+  float* const stx = reinterpret_cast<float*>(smem + SM::off_st);   // pairs: [buf][m][t][lane]
+  float* const flx = reinterpret_cast<float*>(smem + SM::off_fl);
   const uint32_t raw_base = smem_u32(smem + SM::off_raw);
   const uint32_t bar_base = smem_u32(smem + SM::off_bar);
   const uint32_t sync_bar = smem_u32(smem + SM::off_sync);
@@ -260,16 +256,21 @@ __global__ void __launch_bounds__(FNT, 2)
           sy[q] = limited_slope1<LIM>(wc - wpl[q * FS - WPITCH], wpl[q * FS + WPITCH] - wc);
           sz[q] = limited_slope1<LIM>(dLz[q], dRz[q]);
         }
-        // lanes (x, y): the y lane carries (rho, v, w, u, P) so that slot 1 is the normal velocity of both lanes
-        const f2 sxy[5] = {mk2(sx[0], sy[0]), mk2(sx[1], sy[2]), mk2(sx[2], sy[3]), mk2(sx[3], sy[1]), mk2(sx[4], sy[4])};
-        const f2 Wrot[5] = {mk2(Wc[0], Wc[0]), mk2(Wc[1], Wc[2]), mk2(Wc[2], Wc[3]), mk2(Wc[3], Wc[1]), mk2(Wc[4], Wc[4])};
+        // lanes (x, y): the hi lane carries (rho, v, u, w, P) so that slot 1 is the normal velocity of both lanes;
+        // the (z-, z+) pair uses the same two slot orders (slot 3 = w is the normal one in both)
+        const f2 sxy[5] = {mk2(sx[0], sy[0]), mk2(sx[1], sy[2]), mk2(sx[2], sy[1]), mk2(sx[3], sy[3]), mk2(sx[4], sy[4])};
+        const f2 Wrot[5] = {mk2(Wc[0], Wc[0]), mk2(Wc[1], Wc[2]), mk2(Wc[2], Wc[1]), mk2(Wc[3], Wc[3]), mk2(Wc[4], Wc[4])};
         f2 WB[5], WA[5], WC[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
           WB[q] = fma2(c.half, sxy[q], Wrot[q]);     // '+' faces
           WA[q] = fma2(c.halfn, sxy[q], Wrot[q]);    // '-' faces
-          WC[q] = mk2(fmaf(-0.5f, sz[q], Wc[q]), fmaf(0.5f, sz[q], Wc[q]));  // lanes (z-, z+), not rotated
         }
+        WC[0] = mk2(fmaf(-0.5f, sz[0], Wc[0]), fmaf(0.5f, sz[0], Wc[0]));  // lanes (z-, z+)
+        WC[1] = mk2(fmaf(-0.5f, sz[1], Wc[1]), fmaf(0.5f, sz[2], Wc[2]));
+        WC[2] = mk2(fmaf(-0.5f, sz[2], Wc[2]), fmaf(0.5f, sz[1], Wc[1]));
+        WC[3] = mk2(fmaf(-0.5f, sz[3], Wc[3]), fmaf(0.5f, sz[3], Wc[3]));
+        WC[4] = mk2(fmaf(-0.5f, sz[4], Wc[4]), fmaf(0.5f, sz[4], Wc[4]));
         float d[5];
         {
           f2 FB[5], FA[5], FC[5], D[5];
@@ -280,46 +281,41 @@ __global__ void __launch_bounds__(FNT, 2)
           for (int q = 0; q < 5; ++q) D[q] = FB[q] - FA[q];
           const float hl = lo(c.hlamn);
           d[0] = hl * ((lo(D[0]) + hi(D[0])) + (hi(FC[0]) - lo(FC[0])));
-          d[1] = hl * ((lo(D[1]) + hi(D[3])) + (hi(FC[1]) - lo(FC[1])));
-          d[2] = hl * ((lo(D[2]) + hi(D[1])) + (hi(FC[2]) - lo(FC[2])));
-          d[3] = hl * ((lo(D[3]) + hi(D[2])) + (hi(FC[3]) - lo(FC[3])));
+          d[1] = hl * ((lo(D[1]) + hi(D[2])) + (hi(FC[2]) - lo(FC[1])));
+          d[2] = hl * ((lo(D[2]) + hi(D[1])) + (hi(FC[1]) - lo(FC[2])));
+          d[3] = hl * ((lo(D[3]) + hi(D[3])) + (hi(FC[3]) - lo(FC[3])));
           d[4] = hl * ((lo(D[4]) + hi(D[4])) + (hi(FC[4]) - lo(FC[4])));
         }
-        const f2 dUrot[5] = {mk2(d[0], d[0]), mk2(d[1], d[2]), mk2(d[2], d[3]), mk2(d[3], d[1]), mk2(d[4], d[4])};
-        const f2 dUsp[5] = {mk2(d[0], d[0]), mk2(d[1], d[1]), mk2(d[2], d[2]), mk2(d[3], d[3]), mk2(d[4], d[4])};
+        const f2 dUrot[5] = {mk2(d[0], d[0]), mk2(d[1], d[2]), mk2(d[2], d[1]), mk2(d[3], d[3]), mk2(d[4], d[4])};
 
         // ---- B2: the six predicted states; guard; publish x+ / y+
         f2 gmin = c.one;
         {
           const St2 SB = state_from_face(WB, dUrot, c, gmin);
           if (!ghost_plane) {
-            float* xo = xs + buf * (6 * FNT) + t;
-            float* yo = ys + buf * (6 * FNT) + t;
-            xo[0 * FNT] = lo(SB.r); xo[1 * FNT] = lo(SB.u); xo[2 * FNT] = lo(SB.v);
-            xo[3 * FNT] = lo(SB.w); xo[4 * FNT] = lo(SB.p); xo[5 * FNT] = lo(SB.h);
-            yo[0 * FNT] = hi(SB.r); yo[1 * FNT] = hi(SB.u); yo[2 * FNT] = hi(SB.v);
-            yo[3 * FNT] = hi(SB.w); yo[4 * FNT] = hi(SB.p); yo[5 * FNT] = hi(SB.h);
+            float* so = stx + (buf * (6 * FNT) + t) * 2;
+            sts2(so + 0 * (2 * FNT), SB.r); sts2(so + 1 * (2 * FNT), SB.u); sts2(so + 2 * (2 * FNT), SB.v);
+            sts2(so + 3 * (2 * FNT), SB.w); sts2(so + 4 * (2 * FNT), SB.p); sts2(so + 5 * (2 * FNT), SB.h);
           }
         }
         SA = state_from_face(WA, dUrot, c, gmin);
-        St2 SC = state_from_face(WC, dUsp, c, gmin);
+        St2 SC = state_from_face(WC, dUrot, c, gmin);
         if (__builtin_expect(!(lo(gmin) > 0.0f && hi(gmin) > 0.0f), 0)) {
           // rare: first-order fallback (reading R7) — all six states become the cell's own input state
           const float q = fmaf(Wc[3], Wc[3], fmaf(Wc[2], Wc[2], Wc[1] * Wc[1]));
           const float h = fmaf(0.5f, q, (lo(c.gg1) * Wc[4]) * rcp1(Wc[0]));
-          SA.r = mk2(Wc[0], Wc[0]); SA.u = mk2(Wc[1], Wc[2]); SA.v = mk2(Wc[2], Wc[3]); SA.w = mk2(Wc[3], Wc[1]);
+          SA.r = mk2(Wc[0], Wc[0]); SA.u = mk2(Wc[1], Wc[2]); SA.v = mk2(Wc[2], Wc[1]); SA.w = mk2(Wc[3], Wc[3]);
           SA.p = mk2(Wc[4], Wc[4]); SA.h = mk2(h, h);
-          SC.r = SA.r; SC.u = mk2(Wc[1], Wc[1]); SC.v = mk2(Wc[2], Wc[2]); SC.w = mk2(Wc[3], Wc[3]); SC.p = SA.p; SC.h = SA.h;
+          SC = SA;
           if (!ghost_plane) {
-            float* xo = xs + buf * (6 * FNT) + t;
-            float* yo = ys + buf * (6 * FNT) + t;
-            xo[0 * FNT] = Wc[0]; xo[1 * FNT] = Wc[1]; xo[2 * FNT] = Wc[2]; xo[3 * FNT] = Wc[3]; xo[4 * FNT] = Wc[4]; xo[5 * FNT] = h;
-            yo[0 * FNT] = Wc[0]; yo[1 * FNT] = Wc[2]; yo[2 * FNT] = Wc[3]; yo[3 * FNT] = Wc[1]; yo[4 * FNT] = Wc[4]; yo[5 * FNT] = h;
+            float* so = stx + (buf * (6 * FNT) + t) * 2;
+            sts2(so + 0 * (2 * FNT), SA.r); sts2(so + 1 * (2 * FNT), SA.u); sts2(so + 2 * (2 * FNT), SA.v);
+            sts2(so + 3 * (2 * FNT), SA.w); sts2(so + 4 * (2 * FNT), SA.p); sts2(so + 5 * (2 * FNT), SA.h);
           }
           n_guard += 1u;  // every cell that gets here is one whose states are used
         }
         zm = lane_lo(SC);
-        zp = lane_hi(SC);
+        zp = St1{hi(SC.r), hi(SC.v), hi(SC.u), hi(SC.w), hi(SC.p), hi(SC.h)};  // hi lane: slots (v, u, w)
       }
       // everything the neighbours need from this thread is published: arrive, then the z face (needs no neighbour)
       cta_arrive();
@@ -340,15 +336,16 @@ __global__ void __launch_bounds__(FNT, 2)
 
       // ---- E: conservative update of plane k-1 (its x / y fluxes were published one phase earlier)
       if (interior && k >= 1) {
-        const float* fxb = fxs + (buf ^ 1) * (5 * FNT) + t_xr;
-        const float* fyb = fys + (buf ^ 1) * (5 * FNT) + t_yu;
+        const float* fxb = flx + ((buf ^ 1) * (5 * FNT) + t_xr) * 2;      // lane lo: Fx of the upper x neighbour
+        const float* fyb = flx + ((buf ^ 1) * (5 * FNT) + t_yu) * 2 + 1;  // lane hi: Fy (slot order) of the upper y neighbour
         const int us = (int)rs - 3 + ((int)rs < 3 ? DNSTAGE : 0);  // slot of plane k-1 (rs points at plane k+2)
         const float* rawp = reinterpret_cast<const float*>(smem + SM::off_raw + us * SM::raw_stage_bytes) + raw_own;
         float* op = outg + (k - 1) * (FN * FN) + j * FN + i;
         float out[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          out[q] = fmaf(-c.lam, (fxb[q * FNT] + fyb[q * FNT]) + accd[q], rawp[q * (FS * FS)]);
+          const int qs = (q == 1) ? 2 : (q == 2 ? 1 : q);  // slot of global component q in the y lane
+          out[q] = fmaf(-c.lam, (fxb[q * (2 * FNT)] + fyb[qs * (2 * FNT)]) + accd[q], rawp[q * (FS * FS)]);
           op[(size_t)q * (FN * FN * FN)] = out[q];
         }
         const float m2 = fmaf(out[3], out[3], fmaf(out[2], out[2], out[1] * out[1]));
@@ -356,21 +353,20 @@ __global__ void __launch_bounds__(FNT, 2)
       }
       // ---- D: Roe fluxes at the lower x face (lane x) and the lower y face (lane y) of plane k, one packed solve
       if (!ghost_plane) {
-        const float* xl = xs + buf * (6 * FNT) + t_xl;
-        const float* yl = ys + buf * (6 * FNT) + t_yl;
+        const float* xl = stx + (buf * (6 * FNT) + t_xl) * 2;      // lane lo of the lower x neighbour's pair
+        const float* yl = stx + (buf * (6 * FNT) + t_yl) * 2 + 1;  // lane hi of the lower y neighbour's pair
         St2 L;
-        L.r = mk2(xl[0 * FNT], yl[0 * FNT]); L.u = mk2(xl[1 * FNT], yl[1 * FNT]); L.v = mk2(xl[2 * FNT], yl[2 * FNT]);
-        L.w = mk2(xl[3 * FNT], yl[3 * FNT]); L.p = mk2(xl[4 * FNT], yl[4 * FNT]); L.h = mk2(xl[5 * FNT], yl[5 * FNT]);
+        L.r = mk2(xl[0 * (2 * FNT)], yl[0 * (2 * FNT)]); L.u = mk2(xl[1 * (2 * FNT)], yl[1 * (2 * FNT)]);
+        L.v = mk2(xl[2 * (2 * FNT)], yl[2 * (2 * FNT)]); L.w = mk2(xl[3 * (2 * FNT)], yl[3 * (2 * FNT)]);
+        L.p = mk2(xl[4 * (2 * FNT)], yl[4 * (2 * FNT)]); L.h = mk2(xl[5 * (2 * FNT)], yl[5 * (2 * FNT)]);
         f2 F[5];
         roe2<0>(L, SA, c, F);
-        // lane x is in global component order; lane y comes back as (rho, my, mz, mx, E)
-        const float Fy[5] = {hi(F[0]), hi(F[3]), hi(F[1]), hi(F[2]), hi(F[4])};
-        float* fxo = fxs + buf * (5 * FNT) + t;
-        float* fyo = fys + buf * (5 * FNT) + t;
+        // lane x is in global component order; lane y comes back as (rho, my, mx, mz, E)
+        const float Fy[5] = {hi(F[0]), hi(F[2]), hi(F[1]), hi(F[3]), hi(F[4])};
+        float* fo = flx + (buf * (5 * FNT) + t) * 2;
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          fxo[q * FNT] = lo(F[q]);
-          fyo[q * FNT] = Fy[q];
+          sts2(fo + q * (2 * FNT), F[q]);
           accd[q] = (lo(F[q]) + Fy[q]) + Fz[q];  // sum of the lower-face fluxes of plane k
         }
         if (bfg) {  // a5: outer faces of this plane
