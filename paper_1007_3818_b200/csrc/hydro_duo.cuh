@@ -135,20 +135,21 @@ __global__ void __launch_bounds__(FNT, 2)
   const bool in_x = (i >= 0 && i < FN), in_y = (j >= 0 && j < FN), interior = in_x && in_y;
   auto tid_of = [](int ii, int jj) { return jj < 0 ? 288 + ii : (jj >= FN ? 304 + ii : jj * 18 + ii + 1); };
   // the extra cell this thread also converts (layer-2 ghost behind a first-layer ghost; inner corners)
-  int ei = i, ej = j;
-  bool has_extra = true;
-  if (i == -1) ei = -2;
-  else if (i == FN) ei = FN + 1;
-  else if (j == -1) ej = -2;
-  else if (j == FN) ej = FN + 1;
-  else if ((i == 0 || i == FN - 1) && (j == 0 || j == FN - 1)) { ei = (i == 0) ? -1 : FN; ej = (j == 0) ? -1 : FN; }
-  else has_extra = false;
+  // (its offsets are recomputed where used: registers are scarcer than integer instructions here)
+  const bool corner_owner = (i == 0 || i == FN - 1) && (j == 0 || j == FN - 1);
+  const bool has_extra = !interior || corner_owner;
+  auto extra_cell = [&](int& ei, int& ej) {
+    ei = i; ej = j;
+    if (i == -1) ei = -2;
+    else if (i == FN) ei = FN + 1;
+    else if (j == -1) ej = -2;
+    else if (j == FN) ej = FN + 1;
+    else { ei = (i == 0) ? -1 : FN; ej = (j == 0) ? -1 : FN; }
+  };
   const int raw_own = (j + 2) * FS + (i + 2);            // [q][r][c] dense, + q*400
-  const int raw_ext = (ej + 2) * FS + (ei + 2);
   const int w_own = (j + 2) * WPITCH + (i + 2);          // [r][q][c], + q*20
-  const int w_ext = (ej + 2) * WPITCH + (ei + 2);
-  const int t_xl = t > 0 ? t - 1 : 0;                    // thread (i-1, j): same row
-  const int t_xr = t + 1 < FNT ? t + 1 : t;              // thread (i+1, j)
+  // x neighbours in the exchange arrays are threads t -+ 1 (same row): immediate offsets. For the lanes whose x face
+  // is never used (i = -1; the ghost rows) these read an unrelated but valid shared-memory word.
   const int t_yl = in_x ? tid_of(i, j - 1 < -1 ? -1 : j - 1) : t;   // thread (i, j-1)
   const int t_yu = in_x ? tid_of(i, j + 1 > FN ? FN : j + 1) : t;   // thread (i, j+1)
   const bool do_x = in_y && i >= 0;                      // owns the face (i-1/2, j), i in [0,16]
@@ -223,8 +224,9 @@ __global__ void __launch_bounds__(FNT, 2)
       const int buf = k & 1;
       const bool ghost_plane = (k < 0 || k >= FN);
       // ---- A: primitives of plane k+1 (own cell + the layer-2 / corner ghost this thread is responsible for)
-      float Wp[5], dRz[5];
+      float dRz[5];
       {
+        float Wp[5];
         const float* raw = next_plane();
         convert(raw, raw_own, Wp);
         float* wnext = wring + (buf ^ 1) * SM::w_plane;
@@ -233,10 +235,13 @@ __global__ void __launch_bounds__(FNT, 2)
           for (int q = 0; q < 5; ++q) wnext[w_own + q * FS] = Wp[q];
         }
         if (has_extra && k + 1 >= 0 && k + 1 < FN) {
+          int ei, ej;
+          extra_cell(ei, ej);
           float We[5];
-          convert(raw, raw_ext, We);
+          convert(raw, (ej + 2) * FS + (ei + 2), We);
+          float* we = wnext + (ej + 2) * WPITCH + (ei + 2);
 #pragma unroll
-          for (int q = 0; q < 5; ++q) wnext[w_ext + q * FS] = We[q];
+          for (int q = 0; q < 5; ++q) we[q * FS] = We[q];
         }
 #pragma unroll
         for (int q = 0; q < 5; ++q) dRz[q] = Wp[q] - Wc[q];
@@ -336,7 +341,7 @@ __global__ void __launch_bounds__(FNT, 2)
 
       // ---- E: conservative update of plane k-1 (its x / y fluxes were published one phase earlier)
       if (interior && k >= 1) {
-        const float* fxb = flx + ((buf ^ 1) * (5 * FNT) + t_xr) * 2;      // lane lo: Fx of the upper x neighbour
+        const float* fxb = flx + ((buf ^ 1) * (5 * FNT) + t) * 2 + 2;      // lane lo: Fx of the upper x neighbour
         const float* fyb = flx + ((buf ^ 1) * (5 * FNT) + t_yu) * 2 + 1;  // lane hi: Fy (slot order) of the upper y neighbour
         const int us = (int)rs - 3 + ((int)rs < 3 ? DNSTAGE : 0);  // slot of plane k-1 (rs points at plane k+2)
         const float* rawp = reinterpret_cast<const float*>(smem + SM::off_raw + us * SM::raw_stage_bytes) + raw_own;
@@ -353,7 +358,7 @@ __global__ void __launch_bounds__(FNT, 2)
       }
       // ---- D: Roe fluxes at the lower x face (lane x) and the lower y face (lane y) of plane k, one packed solve
       if (!ghost_plane) {
-        const float* xl = stx + (buf * (6 * FNT) + t_xl) * 2;      // lane lo of the lower x neighbour's pair
+        const float* xl = stx + (buf * (6 * FNT) + t) * 2 - 2;      // lane lo of the lower x neighbour's pair
         const float* yl = stx + (buf * (6 * FNT) + t_yl) * 2 + 1;  // lane hi of the lower y neighbour's pair
         St2 L;
         L.r = mk2(xl[0 * (2 * FNT)], yl[0 * (2 * FNT)]); L.u = mk2(xl[1 * (2 * FNT)], yl[1 * (2 * FNT)]);
@@ -380,8 +385,11 @@ __global__ void __launch_bounds__(FNT, 2)
           }
         }
       }
+      if (k < FN) {  // next plane: W(k+1) was published above, so neither it nor the z difference stays in registers
+        const float* wn = wring + (buf ^ 1) * SM::w_plane + w_own;
 #pragma unroll
-      for (int q = 0; q < 5; ++q) { Wc[q] = Wp[q]; dLz[q] = dRz[q]; }
+        for (int q = 0; q < 5; ++q) { const float wp = wn[q * FS]; dLz[q] = wp - Wc[q]; Wc[q] = wp; }
+      }
     }
   }
 
