@@ -31,6 +31,11 @@ struct DuoSmem {
   static constexpr int total = off_sync + 16;
 };
 
+// overwrite a packed register in place (the operand is read-write, so no new register is allocated)
+__device__ __forceinline__ void set2(f2& d, float a, float b) {
+  asm volatile("mov.b64 %0, {%1, %2};" : "+l"(d.v) : "f"(a), "f"(b));
+}
+
 // scalar state for the z-face solve
 struct St1 {
   float r, u, v, w, p, h;
@@ -309,9 +314,12 @@ __global__ void __launch_bounds__(FNT, 2)
           // rare: first-order fallback (reading R7) — all six states become the cell's own input state
           const float q = fmaf(Wc[3], Wc[3], fmaf(Wc[2], Wc[2], Wc[1] * Wc[1]));
           const float h = fmaf(0.5f, q, (lo(c.gg1) * Wc[4]) * rcp1(Wc[0]));
-          SA.r = mk2(Wc[0], Wc[0]); SA.u = mk2(Wc[1], Wc[2]); SA.v = mk2(Wc[2], Wc[1]); SA.w = mk2(Wc[3], Wc[3]);
-          SA.p = mk2(Wc[4], Wc[4]); SA.h = mk2(h, h);
-          SC = SA;
+          // overwritten IN PLACE (read-write asm operands): otherwise the compiler resolves the merge of the two
+          // definitions with two dozen register copies on the hot path
+          set2(SA.r, Wc[0], Wc[0]); set2(SA.u, Wc[1], Wc[2]); set2(SA.v, Wc[2], Wc[1]); set2(SA.w, Wc[3], Wc[3]);
+          set2(SA.p, Wc[4], Wc[4]); set2(SA.h, h, h);
+          set2(SC.r, Wc[0], Wc[0]); set2(SC.u, Wc[1], Wc[2]); set2(SC.v, Wc[2], Wc[1]); set2(SC.w, Wc[3], Wc[3]);
+          set2(SC.p, Wc[4], Wc[4]); set2(SC.h, h, h);
           if (!ghost_plane) {
             float* so = stx + (buf * (6 * FNT) + t) * 2;
             sts2(so + 0 * (2 * FNT), SA.r); sts2(so + 1 * (2 * FNT), SA.u); sts2(so + 2 * (2 * FNT), SA.v);
