@@ -258,18 +258,22 @@ __global__ void __launch_bounds__(FNT, 2)
       if (do_pred) {
         // ---- B1: slopes, face values, own-direction fluxes -> dU
         const float* wpl = wring + buf * SM::w_plane + w_own;
-        float sx[5], sy[5], sz[5];
-#pragma unroll
-        for (int q = 0; q < 5; ++q) {
-          const float wc = Wc[q];
-          sx[q] = limited_slope1<LIM>(wc - wpl[q * FS - 1], wpl[q * FS + 1] - wc);
-          sy[q] = limited_slope1<LIM>(wc - wpl[q * FS - WPITCH], wpl[q * FS + WPITCH] - wc);
-          sz[q] = limited_slope1<LIM>(dLz[q], dRz[q]);
-        }
         // lanes (x, y): the hi lane carries (rho, v, u, w, P) so that slot 1 is the normal velocity of both lanes;
         // the (z-, z+) pair uses the same two slot orders (slot 3 = w is the normal one in both)
-        const f2 sxy[5] = {mk2(sx[0], sy[0]), mk2(sx[1], sy[2]), mk2(sx[2], sy[1]), mk2(sx[3], sy[3]), mk2(sx[4], sy[4])};
         const f2 Wrot[5] = {mk2(Wc[0], Wc[0]), mk2(Wc[1], Wc[2]), mk2(Wc[2], Wc[1]), mk2(Wc[3], Wc[3]), mk2(Wc[4], Wc[4])};
+        f2 sxy[5];
+        float sz[5];
+        {
+          constexpr int QY[5] = {0, 2, 1, 3, 4};  // component held by the hi lane of slot q
+#pragma unroll
+          for (int q = 0; q < 5; ++q) {
+            const int qy = QY[q];
+            const f2 dL = Wrot[q] - mk2(wpl[q * FS - 1], wpl[qy * FS - WPITCH]);   // one-sided differences, both lanes
+            const f2 dR = mk2(wpl[q * FS + 1], wpl[qy * FS + WPITCH]) - Wrot[q];
+            sxy[q] = mk2(limited_slope1<LIM>(lo(dL), lo(dR)), limited_slope1<LIM>(hi(dL), hi(dR)));
+            sz[q] = limited_slope1<LIM>(dLz[q], dRz[q]);
+          }
+        }
         f2 WB[5], WA[5], WC[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
