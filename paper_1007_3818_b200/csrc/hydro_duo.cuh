@@ -140,16 +140,13 @@ __global__ void __launch_bounds__(FNT, 2)
   const bool in_x = (i >= 0 && i < FN), in_y = (j >= 0 && j < FN), interior = in_x && in_y;
   auto tid_of = [](int ii, int jj) { return jj < 0 ? 288 + ii : (jj >= FN ? 304 + ii : jj * 18 + ii + 1); };
   // the extra cell this thread also converts (layer-2 ghost behind a first-layer ghost; inner corners)
-  // (its offsets are recomputed where used: registers are scarcer than integer instructions here)
-  const bool corner_owner = (i == 0 || i == FN - 1) && (j == 0 || j == FN - 1);
-  const bool has_extra = !interior || corner_owner;
-  auto extra_cell = [&](int& ei, int& ej) {
-    ei = i; ej = j;
-    if (i == -1) ei = -2;
-    else if (i == FN) ei = FN + 1;
-    else if (j == -1) ej = -2;
-    else if (j == FN) ej = FN + 1;
-    else { ei = (i == 0) ? -1 : FN; ej = (j == 0) ? -1 : FN; }
+  // The 68 cells of a plane that are only ever neighbours (layer-2 ghosts, inner corners) are converted by warp 9
+  // alone (the ghost rows: the lightest warp), three per lane, instead of by the lanes next to them in every warp.
+  // Extra e = lane + 32 r, r = 0..2: rows -2 / 17 (e < 32), columns -2 / 17 (e < 64), corners (e < 68).
+  auto extra_cell = [&](int e, int& ei, int& ej) {
+    if (e < 32) { ei = e & 15; ej = (e < 16) ? -2 : FN + 1; }
+    else if (e < 64) { ej = e & 15; ei = (e < 48) ? -2 : FN + 1; }
+    else { ei = (e & 1) ? FN : -1; ej = (e & 2) ? FN : -1; }
   };
   const int raw_own = (j + 2) * FS + (i + 2);            // [q][r][c] dense, + q*400
   const int w_own = (j + 2) * WPITCH + (i + 2);          // [r][q][c], + q*20
@@ -239,14 +236,20 @@ __global__ void __launch_bounds__(FNT, 2)
 #pragma unroll
           for (int q = 0; q < 5; ++q) wnext[w_own + q * FS] = Wp[q];
         }
-        if (has_extra && k + 1 >= 0 && k + 1 < FN) {
-          int ei, ej;
-          extra_cell(ei, ej);
-          float We[5];
-          convert(raw, (ej + 2) * FS + (ei + 2), We);
-          float* we = wnext + (ej + 2) * WPITCH + (ei + 2);
+        if (t >= 288 && k + 1 >= 0 && k + 1 < FN) {  // warp 9 (warp-uniform)
 #pragma unroll
-          for (int q = 0; q < 5; ++q) we[q * FS] = We[q];
+          for (int r = 0; r < 3; ++r) {
+            const int e = (t - 288) + 32 * r;
+            if (e < 68) {
+              int ei, ej;
+              extra_cell(e, ei, ej);
+              float We[5];
+              convert(raw, (ej + 2) * FS + (ei + 2), We);
+              float* we = wnext + (ej + 2) * WPITCH + (ei + 2);
+#pragma unroll
+              for (int q = 0; q < 5; ++q) we[q * FS] = We[q];
+            }
+          }
         }
 #pragma unroll
         for (int q = 0; q < 5; ++q) dRz[q] = Wp[q] - Wc[q];
