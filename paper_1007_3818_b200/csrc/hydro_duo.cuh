@@ -351,6 +351,11 @@ __global__ void __launch_bounds__(FNT, 2)
         }
       }
       zplus = zp;
+      if (k < FN) {  // (own data, so still before the wait) next plane: W(k+1) was published above, so neither it nor the z difference stays in registers
+        const float* wn = wring + (buf ^ 1) * SM::w_plane + w_own;
+#pragma unroll
+        for (int q = 0; q < 5; ++q) { const float wp = wn[q * FS]; dLz[q] = wp - Wc[q]; Wc[q] = wp; }
+      }
       cta_wait();  // x+ / y+ states of plane k, primitives of plane k+1, fluxes of plane k-1 visible
       if (t == 0) issue_upto(seq0 + k + 1 + DNSTAGE);
 
@@ -400,11 +405,7 @@ __global__ void __launch_bounds__(FNT, 2)
           }
         }
       }
-      if (k < FN) {  // next plane: W(k+1) was published above, so neither it nor the z difference stays in registers
-        const float* wn = wring + (buf ^ 1) * SM::w_plane + w_own;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) { const float wp = wn[q * FS]; dLz[q] = wp - Wc[q]; Wc[q] = wp; }
-      }
+
     }
   }
 
