@@ -146,7 +146,7 @@ def main():
     ap.add_argument("--ref-groups", type=int, default=64)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused", "fused_scalar", "fused_duo"],
+    ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused", "fused_scalar", "fused_pair"],
                     help="kernel path forced through gamer_hydro_set_path (default: the library's choice)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -173,7 +173,7 @@ def main():
     G = groups.shape[0]
     cells = G * N ** 3
     gh.gamer_hydro_alloc(G, N, GHOST, 4, local_rank)
-    gh.gamer_hydro_set_path({"auto": 0, "generic": 1, "fused": 2, "fused_scalar": 3, "fused_duo": 4}[args.path])
+    gh.gamer_hydro_set_path({"auto": 0, "generic": 1, "fused": 2, "fused_scalar": 3, "fused_pair": 4}[args.path])
     h_in = torch.from_numpy(groups)
     d_in = h_in.to(dev)
     d_out = torch.empty((G, 5, N, N, N), dtype=torch.float32, device=dev)
@@ -262,9 +262,9 @@ def main():
         pass
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                 "frac": achieved_tf / ALU_PEAK_TFLOPS, "traffic": traffic,
-                "kernel": {"auto": "gh::pair_kernel<MinMod>", "fused": "gh::pair_kernel<MinMod>",
+                "kernel": {"auto": "gh::duo_kernel<MinMod>", "fused": "gh::duo_kernel<MinMod>",
                            "fused_scalar": "gh::fused_kernel<float, MinMod, fast>",
-                           "fused_duo": "gh::duo_kernel<MinMod>",
+                           "fused_pair": "gh::pair_kernel<MinMod>",
                            "generic": "gh::predict_kernel + flux_kernel + update_kernel"}[args.path],
                 "flops_per_cell_update": FLOPS_PER_CELL[w.limiter],
                 "peak_derivation": "148 SM x 128 FP32 lanes x 2 FLOP x 1.965 GHz (sm_max_mhz of MEASURED_PEAKS.json)",

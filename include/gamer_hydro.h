@@ -46,14 +46,16 @@ enum {
 enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1 };
 
 /* kernel selection for gamer_hydro_set_path: AUTO picks FUSED when N == 16, else GENERIC. FUSED is the
- * performance path (fp32: two cells per thread, packed f32x2 arithmetic; fp64: one cell per thread);
- * FUSED_SCALAR forces the one-cell-per-thread fused kernel in fp32 as well (a third implementation for tests). */
+ * performance path (fp32: one cell per thread, the two lanes of every packed f32x2 instruction carry two
+ * directions of the cell; fp64: one cell per thread, scalar). FUSED_SCALAR forces the scalar fused kernel in
+ * fp32 as well and FUSED_PAIR the two-cells-per-thread packed kernel: two more, structurally different,
+ * implementations of the same step (tests, comparisons). */
 enum {
   GAMER_HYDRO_PATH_AUTO = 0,
   GAMER_HYDRO_PATH_GENERIC = 1,
   GAMER_HYDRO_PATH_FUSED = 2,
   GAMER_HYDRO_PATH_FUSED_SCALAR = 3,
-  GAMER_HYDRO_PATH_FUSED_DUO = 4   /* fp32: one cell per thread, f32x2 lanes = two directions of the cell */
+  GAMER_HYDRO_PATH_FUSED_PAIR = 4
 };
 
 /* One-time, idempotent, process-global set-up for `device`: checks the compute capability, raises the

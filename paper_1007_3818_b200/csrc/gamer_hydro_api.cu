@@ -194,7 +194,7 @@ int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int gho
   return 0;
 }
 
-// fp32, one cell per thread with the f32x2 lanes carrying two directions of the cell (hydro_duo.cuh)
+// fp32 performance path: one cell per thread, the f32x2 lanes carry two directions of the cell (hydro_duo.cuh)
 int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
                float gamma, int limiter, cudaStream_t stream) {
   CUtensorMap map;
@@ -214,7 +214,7 @@ int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int 
   return 0;
 }
 
-// fp32 performance path: two cells per thread, packed f32x2 arithmetic (hydro_pair.cuh)
+// fp32, two cells per thread with packed f32x2 arithmetic (hydro_pair.cuh); selectable, not the default
 int launch_pair(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
                 float gamma, int limiter, cudaStream_t stream) {
   CUtensorMap map;
@@ -272,12 +272,12 @@ int step_impl(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost,
   int path = g_state.path;
   if (path == GAMER_HYDRO_PATH_AUTO)
     path = fused_supported<R>(N, ghost) ? GAMER_HYDRO_PATH_FUSED : GAMER_HYDRO_PATH_GENERIC;
-  if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR || path == GAMER_HYDRO_PATH_FUSED_DUO) {
+  if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR || path == GAMER_HYDRO_PATH_FUSED_PAIR) {
     if (!fused_supported<R>(N, ghost)) return GAMER_HYDRO_UNSUPPORTED;
     if constexpr (sizeof(R) == 4) {
-      if (path == GAMER_HYDRO_PATH_FUSED)
+      if (path == GAMER_HYDRO_PATH_FUSED_PAIR)
         return launch_pair(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
-      if (path == GAMER_HYDRO_PATH_FUSED_DUO)
+      if (path == GAMER_HYDRO_PATH_FUSED)
         return launch_duo(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
     }
     return launch_fused<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
@@ -402,7 +402,7 @@ int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonp
 }
 
 int gamer_hydro_set_path(int path) {
-  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_DUO) return GAMER_HYDRO_INVALID_ARG;
+  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_PAIR) return GAMER_HYDRO_INVALID_ARG;
   g_state.path = path;
   return 0;
 }

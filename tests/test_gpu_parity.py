@@ -14,7 +14,7 @@ from paper_1007_3818_b200 import workloads as wl
 pytestmark = pytest.mark.gpu
 G = wl.GAMMA
 TOL32_1, TOL32_10, TOL64 = 1e-4, 1e-3, 1e-11
-PATHS = [gh.PATH_FUSED, gh.PATH_GENERIC, gh.PATH_FUSED_DUO]
+PATHS = [gh.PATH_FUSED, gh.PATH_GENERIC, gh.PATH_FUSED_PAIR, gh.PATH_FUSED_SCALAR]
 
 
 def check(groups, dt, dx, limiter, path, tol, gamma=G, max_excl=pu.MAX_EXCLUDED_FRACTION, ghost=2):
