@@ -129,7 +129,8 @@ __global__ void __launch_bounds__(FNT, 2)
   float* const flx = reinterpret_cast<float*>(smem + SM::off_fl);
   const uint32_t raw_base = smem_u32(smem + SM::off_raw);
   const uint32_t bar_base = smem_u32(smem + SM::off_bar);
-  const uint32_t sync_bar = smem_u32(smem + SM::off_sync);
+  const uint32_t sync_bar = smem_u32(smem + SM::off_sync);       // "states of plane k published"
+  const uint32_t flux_bar = sync_bar + 8;                          // "x / y fluxes of plane k published"
 
   // ---- thread -> cell (i, j) of the cross-shaped footprint (as in hydro_fused.cuh)
   const int t = threadIdx.x;
@@ -177,6 +178,7 @@ __global__ void __launch_bounds__(FNT, 2)
   if (t == 0) {
     for (int s = 0; s < DNSTAGE; ++s) mbar_init(bar_base + 8 * s, 1);
     mbar_init(sync_bar, FNT);
+    mbar_init(flux_bar, FNT);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
@@ -185,6 +187,11 @@ __global__ void __launch_bounds__(FNT, 2)
   uint32_t sync_phase = 0;
   auto cta_arrive = [&]() { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(sync_bar) : "memory"); };
   auto cta_wait = [&]() { mbar_wait(sync_bar, sync_phase); sync_phase ^= 1u; };
+  // second split barrier for the fluxes: its wait (before the update of plane k-1) targets the arrive at the END of the
+  // previous plane, so it is almost always already complete; the first wait passes on the fresh barrier (parity 1)
+  uint32_t flux_phase = 1;
+  auto flux_arrive = [&]() { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(flux_bar) : "memory"); };
+  auto flux_wait = [&]() { mbar_wait(flux_bar, flux_phase); flux_phase ^= 1u; };
   uint32_t rs = 0, rph = 0;  // raw-ring consumer state
   auto next_plane = [&]() -> const float* {
     mbar_wait(bar_base + 8 * rs, rph);
@@ -356,9 +363,7 @@ __global__ void __launch_bounds__(FNT, 2)
 #pragma unroll
         for (int q = 0; q < 5; ++q) { const float wp = wn[q * FS]; dLz[q] = wp - Wc[q]; Wc[q] = wp; }
       }
-      cta_wait();  // x+ / y+ states of plane k, primitives of plane k+1, fluxes of plane k-1 visible
-      if (t == 0) issue_upto(seq0 + k + 1 + DNSTAGE);
-
+      flux_wait();  // x / y fluxes of plane k-1 visible (published before the END of the previous plane)
       // ---- E: conservative update of plane k-1 (its x / y fluxes were published one phase earlier)
       if (interior && k >= 1) {
         const float* fxb = flx + ((buf ^ 1) * (5 * FNT) + t) * 2 + 2;      // lane lo: Fx of the upper x neighbour
@@ -376,6 +381,9 @@ __global__ void __launch_bounds__(FNT, 2)
         const float m2 = fmaf(out[3], out[3], fmaf(out[2], out[2], out[1] * out[1]));
         n_nonpos += (out[0] > 0.0f && (out[0] + out[0]) * out[4] > m2) ? 0u : 1u;
       }
+      cta_wait();  // x+ / y+ states of plane k and primitives of plane k+1 visible
+      if (t == 0) issue_upto(seq0 + k + 1 + DNSTAGE);
+
       // ---- D: Roe fluxes at the lower x face (lane x) and the lower y face (lane y) of plane k, one packed solve
       if (!ghost_plane) {
         const float* xl = stx + (buf * (6 * FNT) + t) * 2 - 2;      // lane lo of the lower x neighbour's pair
@@ -406,6 +414,7 @@ __global__ void __launch_bounds__(FNT, 2)
         }
       }
 
+      flux_arrive();
     }
   }
 
