@@ -204,3 +204,96 @@ def test_mirror_symmetry_gpu():
         back = np.flip(b, axis=4 - axis).copy()
         back[:, 1 + axis] *= -1
         assert metrics.max_rel_err(back, a, G) <= 2e-6
+
+
+def test_cfg4_sedov_blast_fp64_and_fp32():
+    """configs[4] scaled to 64^3 (64 groups), 100 steps at C = 0.4 on the GPU: positivity of rho and P at every
+    step, the Sedov-Taylor radius and exponent of pin P15, fp64 parity with the oracle run on the same dt sequence."""
+    golden = {}
+    import os
+    with open(os.path.join(os.path.dirname(__file__), "golden", "sedov_xi0.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()[:2]
+                golden[k] = float(v)
+    xi0 = golden["gamma_5_3"]
+    n = 64
+    c = (np.arange(n) + 0.5) / n - 0.5
+    R = np.sqrt(c[:, None, None] ** 2 + c[None, :, None] ** 2 + c[None, None, :] ** 2)
+    for dtype in (np.float64, np.float32):
+        w = wl.config_4_sedov(n, steps=100, dtype=dtype)
+        dx = w.dx if dtype == np.float64 else pu.f32(w.dx)
+        radii, times = [], []
+
+        def on_step(i, U, t):
+            U = U.astype(np.float64)
+            assert U[0].min() > 0
+            P = (G - 1) * (U[4] - 0.5 * (U[1] ** 2 + U[2] ** 2 + U[3] ** 2) / U[0])
+            assert P.min() > 0, (dtype, i, P.min())
+            if i + 1 >= 50:
+                shell = U[0] > 1.5
+                radii.append(R[shell].max() if shell.any() else 0.0)
+                times.append(t)
+
+        gpu_step = lambda grp, dt: pu.run_gpu(grp, dt if dtype == np.float64 else pu.f32(dt), dx, G, 0, want_bflux=False)[0]
+        Ug, t, dts = wl.advance(w.U, w.dx, w.bc, 0, w.cfl, w.steps, gpu_step, dtype=dtype, on_step=on_step)
+        R_st = xi0 * (w.meta["E0"] * t * t / 1.0) ** 0.2
+        assert abs(radii[-1] - R_st) <= max(1.5 * w.dx, 0.15 * R_st), (dtype, radii[-1], R_st)
+        slope = np.polyfit(np.log(times), np.log(radii), 1)[0]
+        assert 0.34 <= slope <= 0.46, (dtype, slope)
+        if dtype == np.float64:
+            # the oracle on the same dt sequence: one step within 1e-11, 20 steps within 1e-9 (round-off grows with
+            # the strong shock; north_star fixes only the one-step bound)
+            Uo = w.U.astype(np.float64)
+            Ug1 = None
+            for s, dt in enumerate(dts[:20]):
+                grp = wl.cut_groups(Uo, w.bc)
+                if s == 0:
+                    Ug1 = pu.run_gpu(grp, dt, dx, G, 0, want_bflux=False)[0]
+                r = O.step_groups(grp, 16, 2, dt, dx, G, 0, want_bflux=False, want_guard=False)
+                if s == 0:
+                    assert metrics.max_rel_err(Ug1, r.U_out, G) <= TOL64
+                Uo = wl.assemble_box(r.U_out, w.shape)
+            Ug20, _, _ = wl.advance(w.U, w.dx, w.bc, 0, w.cfl, 20, gpu_step, dtype=dtype)
+            assert metrics.max_rel_err(Ug20[None], Uo[None], G) <= 1e-9
+
+
+def test_headline_full_size_in_the_bench_launch_configuration():
+    """BASELINE.json:configs[3] at FULL size (32768 groups, the batch and launch geometry bench.py times, default
+    kernel path): sampled groups — seeded random ones plus those holding the extreme densities — against the
+    oracle element by element, and properties that hold at any size: finite output everywhere, the per-group flux
+    balance (pin P11) on every group, guard count equal to the oracle's on the sample up to marginal cells."""
+    w = wl.config_3_cosmo(512, seed=3)
+    grp = w.groups()
+    n = grp.shape[0]
+    assert n == 32768
+    dt, dx = pu.f32(w.dt()), pu.f32(w.dx)
+    dev = torch.device("cuda", 0)
+    x = torch.from_numpy(grp).to(dev)
+    out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float32, device=dev)
+    bf = torch.full((n, 6, 5, 16, 16), float("nan"), dtype=torch.float32, device=dev)
+    gh.gamer_hydro_status()
+    gh.gamer_hydro_step(x, out, bf, n, 16, 2, dt, dx, G, w.limiter)
+    torch.cuda.synchronize()
+    guard_gpu, nonpos = gh.gamer_hydro_status()
+    assert bool(torch.isfinite(out).all()) and bool(torch.isfinite(bf).all())
+    # P11 on every group, on the device in fp64: sum(U_out - U_in) = -lambda * (F_hi - F_lo summed over the faces)
+    lam = dt / dx
+    xin = x[:, :, 2:-2, 2:-2, 2:-2].double()
+    dU = (out.double() - xin).sum(dim=(2, 3, 4))
+    b = bf.double().sum(dim=(3, 4))
+    net = (b[:, 1] - b[:, 0]) + (b[:, 3] - b[:, 2]) + (b[:, 5] - b[:, 4])
+    # residual budget: every stored U_out is rounded to fp32 (half an ulp of |U| per cell) and so is every flux
+    budget = 1.2e-7 * xin.abs().sum(dim=(2, 3, 4)) + 1e-5 * lam * bf.double().abs().sum(dim=(1, 3, 4)) + 1e-300
+    assert float(((dU + lam * net).abs() / budget).max()) <= 1.0
+    # sampled groups against the oracle
+    rho_max = grp[:, 0].reshape(n, -1).max(axis=1)
+    rho_min = grp[:, 0].reshape(n, -1).min(axis=1)
+    rng = np.random.default_rng(2026)
+    idx = np.unique(np.concatenate([rng.choice(n, 96, replace=False), [rho_max.argmax(), rho_min.argmin(), 0, n - 1]]))
+    res = pu.compare(grp[idx], dt, dx, G, w.limiter, out[idx].cpu().numpy(), bf[idx].cpu().numpy())
+    assert res["excluded_fraction"] <= 1e-3, res["excluded_fraction"]
+    assert res["err"] <= TOL32_1, res["err"]
+    assert res["err_bflux"] <= 10 * TOL32_1, res["err_bflux"]
+    assert nonpos == 0
+    assert guard_gpu > 0
