@@ -297,3 +297,38 @@ def test_headline_full_size_in_the_bench_launch_configuration():
     assert res["err_bflux"] <= 10 * TOL32_1, res["err_bflux"]
     assert nonpos == 0
     assert guard_gpu > 0
+
+
+@pytest.mark.parametrize("path", [gh.PATH_FUSED, gh.PATH_FUSED_PAIR, gh.PATH_FUSED_SCALAR])
+def test_repeated_launches_are_bit_identical(path):
+    """Race stress for the split-barrier / double-buffer protocols of the fused kernels: 4096 groups (14 per
+    persistent CTA, so every buffer is recycled hundreds of times) launched 25 times must give the same bits every
+    time, for outputs and boundary fluxes, and the same bits as a batch that puts other groups on each CTA."""
+    w = wl.config_3_cosmo(256, seed=5)
+    grp = w.groups()
+    n = grp.shape[0]
+    dt, dx = pu.f32(w.dt()), pu.f32(w.dx)
+    dev = torch.device("cuda", 0)
+    x = torch.from_numpy(grp).to(dev)
+    gh.gamer_hydro_set_path(path)
+    try:
+        ref_out = ref_bf = None
+        for rep in range(25):
+            out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float32, device=dev)
+            bf = torch.full((n, 6, 5, 16, 16), float("nan"), dtype=torch.float32, device=dev)
+            gh.gamer_hydro_step(x, out, bf, n, 16, 2, dt, dx, G, w.limiter)
+            torch.cuda.synchronize()
+            if rep == 0:
+                ref_out, ref_bf = out, bf
+                assert bool(torch.isfinite(out).all()) and bool(torch.isfinite(bf).all())
+            else:
+                assert torch.equal(out.view(torch.int32), ref_out.view(torch.int32)), rep
+                assert torch.equal(bf.view(torch.int32), ref_bf.view(torch.int32)), rep
+        # a different batch (the last 1000 groups only): other CTA / ring-slot assignment, same bits per group
+        m = 1000
+        out = torch.empty((m, 5, 16, 16, 16), dtype=torch.float32, device=dev)
+        gh.gamer_hydro_step(x[n - m:].contiguous(), out, None, m, 16, 2, dt, dx, G, w.limiter)
+        torch.cuda.synchronize()
+        assert torch.equal(out.view(torch.int32), ref_out[n - m:].view(torch.int32))
+    finally:
+        gh.gamer_hydro_set_path(gh.PATH_AUTO)
