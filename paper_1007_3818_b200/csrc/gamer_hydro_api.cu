@@ -86,8 +86,8 @@ int init_locked(int device) {
   if ((rc = set_fused_attr<double, 1, false>())) return rc;
   CK(cudaFuncSetAttribute(gh::pair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
   CK(cudaFuncSetAttribute(gh::pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
-  CK(cudaFuncSetAttribute(gh::duo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DuoSmem::total));
-  CK(cudaFuncSetAttribute(gh::duo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DuoSmem::total));
+  CK(cudaFuncSetAttribute(gh::duo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
+  CK(cudaFuncSetAttribute(gh::duo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
@@ -201,14 +201,13 @@ int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int 
   int rc = encode_plane_map<float>(U_in, n_groups, N, ghost, map);
   if (rc) return rc;
   const gh::PairConst c = gh::make_pair_consts(dt, dx, gamma);
-  const int smem = gh::DuoSmem::total;
-  const int per_sm = (2 * (smem + 1024) <= g_state.smem_per_sm) ? 2 : 1;
-  const int resident = g_state.sm_count * per_sm;
-  const int grid = n_groups < resident ? n_groups : resident;
+  const int smem = gh::DHALVES * gh::DuoSmem::total_padded;   // one CTA per SM: two independent 320-thread halves
+  const int want = (n_groups + gh::DHALVES - 1) / gh::DHALVES;
+  const int grid = want < g_state.sm_count ? want : g_state.sm_count;
   if (limiter == 0)
-    gh::duo_kernel<0><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+    gh::duo_kernel<0><<<grid, gh::FNT * gh::DHALVES, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
   else
-    gh::duo_kernel<1><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+    gh::duo_kernel<1><<<grid, gh::FNT * gh::DHALVES, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   return 0;

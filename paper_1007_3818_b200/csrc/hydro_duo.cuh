@@ -17,6 +17,7 @@
 namespace gh {
 
 constexpr int DNSTAGE = 5;   // raw-plane ring depth
+constexpr int DHALVES = 2;   // independent 320-thread halves per CTA (see duo_kernel)
 
 struct DuoSmem {
   static constexpr int raw_stage_bytes = ((PRAW * 4 + 127) / 128) * 128;
@@ -29,6 +30,7 @@ struct DuoSmem {
   static constexpr int off_bar = ((off_fl + 2 * 5 * FNT * 8 + 15) / 16) * 16;
   static constexpr int off_sync = off_bar + DNSTAGE * 8;
   static constexpr int total = off_sync + 16;
+  static constexpr int total_padded = ((total + 127) / 128) * 128;   // one half-CTA's region
 };
 
 // overwrite a packed register in place (the operand is read-write, so no new register is allocated)
@@ -118,12 +120,22 @@ __device__ __forceinline__ float limited_slope1(float a, float b) {
   return vanleer1(a, b, p, s);
 }
 
-template <int LIM>
-__global__ void __launch_bounds__(FNT, 2)
-    duo_kernel(const __grid_constant__ CUtensorMap in_map, float* __restrict__ U_out, float* __restrict__ bflux,
-               int n_groups, int goff, const __grid_constant__ PairConst c, unsigned long long* __restrict__ status) {
+// One half-CTA (320 threads). HALF is a template parameter so that every shared-memory address and the named
+// barrier id stay compile-time constants: a run-time half offset costs registers this kernel does not have.
+template <int LIM, int HALF>
+__device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __restrict__ U_out, float* __restrict__ bflux,
+                                         int n_groups, int goff, const PairConst& c,
+                                         unsigned long long* __restrict__ status, unsigned char* smem_cta) {
   using SM = DuoSmem;
-  extern __shared__ __align__(128) unsigned char smem[];
+  // The CTA is TWO independent halves of 320 threads (10 warps), each with its own shared-memory region, group
+  // stream, TMA ring and barriers. Why one 20-warp CTA instead of two 10-warp CTAs: a 10-warp CTA puts 3, 3, 2, 2
+  // warps on the four schedulers and the hardware places two such CTAs the same way (6, 6, 4, 4: measured with
+  // clock probes, the warps of the two light schedulers idle 13 % at the barrier); warps 10..19 of one CTA land
+  // on schedulers 2, 3, 0, 1, ... and make it 5, 5, 5, 5.
+  constexpr int half_id = HALF;
+  unsigned char* const smem = smem_cta + HALF * SM::total_padded;
+  const int vblock = (int)blockIdx.x * DHALVES + HALF, vgrid = (int)gridDim.x * DHALVES;
+  auto half_sync = [&]() { asm volatile("bar.sync %0, %1;" ::"n"(1 + HALF), "n"(FNT) : "memory"); };
   float* const wring = reinterpret_cast<float*>(smem + SM::off_w);
   float* const stx = reinterpret_cast<float*>(smem + SM::off_st);   // pairs: [buf][m][t][lane]
   float* const flx = reinterpret_cast<float*>(smem + SM::off_fl);
@@ -133,7 +145,7 @@ __global__ void __launch_bounds__(FNT, 2)
   const uint32_t flux_bar = sync_bar + 8;                          // "x / y fluxes of plane k published"
 
   // ---- thread -> cell (i, j) of the cross-shaped footprint (as in hydro_fused.cuh)
-  const int t = threadIdx.x;
+  const int t = (int)threadIdx.x - half_id * FNT;
   int i, j;
   if (t < 288) { j = t / 18; i = t % 18 - 1; }
   else if (t < 304) { j = -1; i = t - 288; }
@@ -158,10 +170,10 @@ __global__ void __launch_bounds__(FNT, 2)
   const bool do_x = in_y && i >= 0;                      // owns the face (i-1/2, j), i in [0,16]
   const bool do_y = in_x && j >= 0;                      // owns the face (i, j-1/2), j in [0,16]
 
-  const int n_local = (n_groups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
+  const int n_local = (n_groups - vblock + vgrid - 1) / vgrid;
   const int total_planes = n_local * FPLANES;
   // TMA producer state (thread 0 only), kept incrementally
-  int issued = 0, iss_p = 0, iss_g = (int)blockIdx.x;
+  int issued = 0, iss_p = 0, iss_g = vblock;
   uint32_t iss_slot = 0;
   auto issue_upto = [&](int limit) {
     if (limit > total_planes) limit = total_planes;
@@ -171,7 +183,7 @@ __global__ void __launch_bounds__(FNT, 2)
       mbar_expect_tx(bar, SM::raw_tx_bytes);
       tma_load_plane(raw_base + iss_slot * SM::raw_stage_bytes, &in_map, goff, goff, goff + iss_p, iss_g, bar);
       ++issued;
-      if (++iss_p == FPLANES) { iss_p = 0; iss_g += (int)gridDim.x; }
+      if (++iss_p == FPLANES) { iss_p = 0; iss_g += vgrid; }
       if (++iss_slot == DNSTAGE) iss_slot = 0;
     }
   };
@@ -182,7 +194,7 @@ __global__ void __launch_bounds__(FNT, 2)
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
-  __syncthreads();
+  half_sync();
   if (t == 0) issue_upto(DNSTAGE);
   uint32_t sync_phase = 0;
   auto cta_arrive = [&]() { asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(sync_bar) : "memory"); };
@@ -210,7 +222,7 @@ __global__ void __launch_bounds__(FNT, 2)
   unsigned int n_guard = 0, n_nonpos = 0;
 
   for (int it = 0; it < n_local; ++it) {
-    const int g = (int)blockIdx.x + it * (int)gridDim.x;
+    const int g = vblock + it * vgrid;
     const int seq0 = it * FPLANES;
     float* const outg = U_out + (size_t)g * (5 * FN * FN * FN);
     float* const bfg = bflux ? bflux + (size_t)g * (30 * FN * FN) : nullptr;
@@ -226,7 +238,7 @@ __global__ void __launch_bounds__(FNT, 2)
       for (int q = 0; q < 5; ++q) { wpl[w_own + q * FS] = Wc[q]; dLz[q] = Wc[q] - Wm[q]; accd[q] = 1.0f; Fz[q] = 1.0f; }
       zplus = St1{1.0f, 1.0f, 1.0f, 1.0f, 1.0f, 1.0f};
     }
-    __syncthreads();
+    half_sync();
     if (t == 0) issue_upto(seq0 + 2 + DNSTAGE);
 
     for (int k = -1; k <= FN; ++k) {
@@ -426,6 +438,15 @@ __global__ void __launch_bounds__(FNT, 2)
     if (n_guard) atomicAdd(&status[0], (unsigned long long)n_guard);
     if (n_nonpos) atomicAdd(&status[1], (unsigned long long)n_nonpos);
   }
+}
+
+template <int LIM>
+__global__ void __launch_bounds__(FNT * DHALVES, 1)
+    duo_kernel(const __grid_constant__ CUtensorMap in_map, float* __restrict__ U_out, float* __restrict__ bflux,
+               int n_groups, int goff, const __grid_constant__ PairConst c, unsigned long long* __restrict__ status) {
+  extern __shared__ __align__(128) unsigned char smem_cta[];
+  if (threadIdx.x < FNT) duo_half<LIM, 0>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta);
+  else duo_half<LIM, 1>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta);
 }
 
 }  // namespace gh
