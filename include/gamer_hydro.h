@@ -88,6 +88,34 @@ int gamer_hydro_step_f64(const double* U_in_with_ghosts, double* U_out, double* 
 int gamer_hydro_step_host(const float* h_U_in_with_ghosts, float* h_U_out, float* h_boundary_fluxes, int n_groups,
                           int N, int ghost, float dt, float dx, float gamma, int limiter, int chunk_groups);
 
+/* ---- the steps either side of the hot path, for device-resident multi-step runs on ONE uniform grid of
+ * gx x gy x gz patch groups (group index x-fastest: g = (bz * gy + by) * gx + bx). The paper does both on the CPU
+ * ("the operation of preparing the ghost-zone data is conducted by CPU"); here they are plain
+ * streaming kernels so that a run never leaves the GPU. bytes_per_real is 4 or 8. ---- */
+
+/* CFL signal speed (reading R15): *h_max (HOST) = max over the interior cells of all groups of
+ * |vx| + |vy| + |vz| + 3 c_s, c_s = sqrt(gamma max(P, 0) / rho). U is a DEVICE array [n_groups][5][S][S][S],
+ * S = N + 2 ghost (ghost = 0 for a U_out array). Synchronises `stream`. */
+int gamer_hydro_max_speed(const void* U, int bytes_per_real, int n_groups, int N, int ghost, double gamma,
+                          double* h_max, cudaStream_t stream);
+
+/* Same-level ghost-shell refill (reading R16): rebuilds every stored cell of U_in_with_ghosts
+ * [G][5][S][S][S] — interior and ghost shell — from the interior arrays U_out [G][5][N][N][N] of the groups that
+ * own the cells; per axis bc = 0 wraps periodically, bc = 1 copies the nearest interior cell (outflow). Device
+ * pointers, enqueue-and-return; the two arrays must not alias. */
+int gamer_hydro_fill_ghosts(const void* U_out, void* U_in_with_ghosts, int bytes_per_real, int gx, int gy, int gz, int N,
+                            int ghost, int bc_x, int bc_y, int bc_z, cudaStream_t stream);
+
+/* n_steps time steps of the fp32 path on one uniform grid without leaving the device: per step
+ * dt = float(cfl * dx / max signal speed) (fp64 on the host from the device-side maximum, R15/R11), then
+ * gamer_hydro_step, then gamer_hydro_fill_ghosts. U (ghost shells filled on entry) holds the final state with
+ * refilled ghost shells on return, U_out the interiors of the last step, boundary_fluxes (may be NULL) those of
+ * the last step; h_dts (HOST, n_steps floats, may be NULL) receives the time steps taken. One 4-byte
+ * device-to-host read and one stream synchronisation per step. */
+int gamer_hydro_advance(float* U_with_ghosts, float* U_out, float* boundary_fluxes, int gx, int gy, int gz, int N,
+                        int ghost, int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dx, float gamma,
+                        int limiter, float* h_dts, cudaStream_t stream);
+
 /* Diagnostics accumulated since the last call (and reset by it): number of cells whose predicted face
  * states failed the positivity guard and fell back to first order (R7), and number of updated
  * cells with rho <= 0 or P <= 0 (R10: counted, never floored). Synchronises the device. Either pointer may

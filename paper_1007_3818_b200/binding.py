@@ -19,7 +19,8 @@ PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_PAIR = 0, 1, 
 
 EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
-           "gamer_hydro_strerror"]
+           "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance"]
+BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
 class GamerHydroError(RuntimeError):
@@ -42,6 +43,9 @@ def lib():
         L.gamer_hydro_step_host.argtypes = [vp, vp, vp, i, i, i, f, f, f, i, i]
         L.gamer_hydro_status.argtypes = [C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.gamer_hydro_set_path.argtypes = [i]
+        L.gamer_hydro_max_speed.argtypes = [vp, i, i, i, i, d, C.POINTER(C.c_double), vp]
+        L.gamer_hydro_fill_ghosts.argtypes = [vp, vp, i, i, i, i, i, i, i, i, i, vp]
+        L.gamer_hydro_advance.argtypes = [vp, vp, vp, i, i, i, i, i, i, i, i, i, f, f, f, i, vp, vp]
         L.gamer_hydro_launch_count.restype = C.c_ulonglong
         L.gamer_hydro_strerror.restype = C.c_char_p
         L.gamer_hydro_strerror.argtypes = [i]
@@ -116,6 +120,55 @@ def gamer_hydro_step_host(h_U_in, h_U_out, h_boundary_fluxes, n_groups=None, N=1
     _check(lib().gamer_hydro_step_host(h_U_in.data_ptr(), h_U_out.data_ptr(), bf, G, N, ghost, dt, dx, gamma,
                                        int(limiter), int(chunk_groups)))
     return h_U_out
+
+
+def _real_bytes(x):
+    if not (x.is_cuda and x.is_contiguous() and x.dtype in (torch.float32, torch.float64)):
+        raise GamerHydroError("tensors must be contiguous CUDA tensors of dtype float32 or float64")
+    return 4 if x.dtype == torch.float32 else 8
+
+
+def gamer_hydro_max_speed(U, N=16, ghost=2, gamma=5.0 / 3.0, stream=None):
+    """max over the interior cells of |vx|+|vy|+|vz|+3 c_s (R15) of a device array [G][5][S][S][S]; synchronises."""
+    S = N + 2 * ghost
+    if U.dim() != 5 or tuple(U.shape[1:]) != (5, S, S, S):
+        raise GamerHydroError("U must be [n_groups][5][%d][%d][%d]" % (S, S, S))
+    out = C.c_double(0.0)
+    _check(lib().gamer_hydro_max_speed(U.data_ptr(), _real_bytes(U), U.shape[0], N, ghost, gamma, C.byref(out),
+                                       _stream_ptr(stream)))
+    return float(out.value)
+
+
+def gamer_hydro_fill_ghosts(U_out, U_in_with_ghosts, grid, N=16, ghost=2, bc=(BC_PERIODIC,) * 3, stream=None):
+    """Rebuilds U_in_with_ghosts [G][5][S][S][S] from the interiors U_out [G][5][N][N][N] of one uniform grid of
+    grid = (gx, gy, gz) groups (x-fastest group index); bc per axis: BC_PERIODIC or BC_OUTFLOW (R16)."""
+    gx, gy, gz = (int(v) for v in grid)
+    G, S = gx * gy * gz, N + 2 * ghost
+    if tuple(U_out.shape) != (G, 5, N, N, N) or tuple(U_in_with_ghosts.shape) != (G, 5, S, S, S):
+        raise GamerHydroError("shapes do not match a %dx%dx%d grid of groups" % (gx, gy, gz))
+    if _real_bytes(U_out) != _real_bytes(U_in_with_ghosts):
+        raise GamerHydroError("U_out and U_in_with_ghosts must have the same dtype")
+    _check(lib().gamer_hydro_fill_ghosts(U_out.data_ptr(), U_in_with_ghosts.data_ptr(), _real_bytes(U_out), gx, gy, gz,
+                                         N, ghost, int(bc[0]), int(bc[1]), int(bc[2]), _stream_ptr(stream)))
+    return U_in_with_ghosts
+
+
+def gamer_hydro_advance(U_with_ghosts, U_out, boundary_fluxes, grid, n_steps, cfl, dx, N=16, ghost=2,
+                        bc=(BC_PERIODIC,) * 3, gamma=5.0 / 3.0, limiter=MINMOD, stream=None):
+    """n_steps fp32 steps on one uniform grid without leaving the device; returns the list of time steps taken."""
+    gx, gy, gz = (int(v) for v in grid)
+    G, S = gx * gy * gz, N + 2 * ghost
+    if tuple(U_with_ghosts.shape) != (G, 5, S, S, S) or tuple(U_out.shape) != (G, 5, N, N, N):
+        raise GamerHydroError("shapes do not match a %dx%dx%d grid of groups" % (gx, gy, gz))
+    for x in (U_with_ghosts, U_out, boundary_fluxes):
+        if x is not None and not (x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()):
+            raise GamerHydroError("tensors must be contiguous CUDA float32 tensors")
+    dts = (C.c_float * max(int(n_steps), 1))()
+    bf = boundary_fluxes.data_ptr() if boundary_fluxes is not None else None
+    _check(lib().gamer_hydro_advance(U_with_ghosts.data_ptr(), U_out.data_ptr(), bf, gx, gy, gz, N, ghost, int(bc[0]),
+                                     int(bc[1]), int(bc[2]), int(n_steps), cfl, dx, gamma, int(limiter), dts,
+                                     _stream_ptr(stream)))
+    return [float(dts[s]) for s in range(int(n_steps))]
 
 
 def gamer_hydro_status():

@@ -15,6 +15,7 @@
 #include "hydro_generic.cuh"
 #include "hydro_pair.cuh"
 #include "hydro_duo.cuh"
+#include "hydro_aux.cuh"
 
 namespace {
 
@@ -77,8 +78,9 @@ int init_locked(int device) {
   CK(cudaSetDevice(device));
   g_state.sm_count = prop.multiProcessorCount;
   g_state.smem_per_sm = (int)prop.sharedMemPerMultiprocessor;
-  CK(cudaMalloc(&g_state.status, 2 * sizeof(unsigned long long)));
-  CK(cudaMemset(g_state.status, 0, 2 * sizeof(unsigned long long)));
+  // [0] guard cells, [1] non-positive outputs, [2] bit pattern of the running signal-speed maximum
+  CK(cudaMalloc(&g_state.status, 4 * sizeof(unsigned long long)));
+  CK(cudaMemset(g_state.status, 0, 4 * sizeof(unsigned long long)));
   int rc;
   if ((rc = set_fused_attr<float, 0, true>())) return rc;
   if ((rc = set_fused_attr<float, 1, true>())) return rc;
@@ -296,6 +298,55 @@ void free_host_bufs() {
 
 }  // namespace
 
+namespace {
+
+template <class R, class Bits>
+int max_speed_impl(const R* U, int n_groups, int N, int ghost, double gamma, double* h_max, cudaStream_t stream) {
+  if (!U || !h_max || n_groups < 0 || N < 1 || ghost < 0 || !(gamma > 1.0)) return GAMER_HYDRO_INVALID_ARG;
+  *h_max = 0.0;
+  if (n_groups == 0) return 0;
+  int rc = ensure_init();
+  if (rc) return rc;
+  Bits* slot = reinterpret_cast<Bits*>(g_state.status + 2);
+  CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
+  const long long n_cells = (long long)n_groups * N * N * N;
+  const int threads = 256;
+  long long want = (n_cells + threads - 1) / threads;
+  const int grid = (int)(want < (long long)g_state.sm_count * 16 ? want : (long long)g_state.sm_count * 16);
+  gh::max_speed_kernel<R, Bits><<<grid, threads, 0, stream>>>(U, n_cells, N, ghost, (R)gamma, slot);
+  g_launches.fetch_add(1);
+  CK(cudaGetLastError());
+  Bits bits = 0;
+  CK(cudaMemcpyAsync(&bits, slot, sizeof(Bits), cudaMemcpyDeviceToHost, stream));
+  CK(cudaStreamSynchronize(stream));
+  R v;
+  memcpy(&v, &bits, sizeof(R));
+  *h_max = (double)v;
+  return 0;
+}
+
+template <class R>
+int fill_ghosts_impl(const R* U_out, R* U_in, int gx, int gy, int gz, int N, int ghost, int bcx, int bcy, int bcz,
+                     cudaStream_t stream) {
+  if (!U_out || !U_in || gx < 1 || gy < 1 || gz < 1 || N < 1 || ghost < 0 || (bcx | bcy | bcz) < 0 || bcx > 1 ||
+      bcy > 1 || bcz > 1)
+    return GAMER_HYDRO_INVALID_ARG;
+  if ((long long)gx * gy * gz > 0x7fffffffLL) return GAMER_HYDRO_INVALID_ARG;
+  int rc = ensure_init();
+  if (rc) return rc;
+  const int S = N + 2 * ghost;
+  const long long total = (long long)gx * gy * gz * S * S * S;
+  const int threads = 256;
+  long long want = (total + threads - 1) / threads;
+  const int grid = (int)(want < (long long)g_state.sm_count * 32 ? want : (long long)g_state.sm_count * 32);
+  gh::fill_ghosts_kernel<R><<<grid, threads, 0, stream>>>(U_out, U_in, gx, gy, gz, N, ghost, bcx, bcy, bcz);
+  g_launches.fetch_add(1);
+  CK(cudaGetLastError());
+  return 0;
+}
+
+}  // namespace
+
 extern "C" {
 
 int gamer_hydro_alloc(int max_groups, int N, int ghost, int bytes_per_real, int device) {
@@ -340,6 +391,44 @@ int gamer_hydro_step(const float* U_in, float* U_out, float* bflux, int n_groups
 int gamer_hydro_step_f64(const double* U_in, double* U_out, double* bflux, int n_groups, int N, int ghost, double dt,
                          double dx, double gamma, int limiter, cudaStream_t stream) {
   return step_impl<double>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+}
+
+int gamer_hydro_max_speed(const void* U, int bytes_per_real, int n_groups, int N, int ghost, double gamma,
+                          double* h_max, cudaStream_t stream) {
+  if (bytes_per_real == 4)
+    return max_speed_impl<float, unsigned int>((const float*)U, n_groups, N, ghost, gamma, h_max, stream);
+  if (bytes_per_real == 8)
+    return max_speed_impl<double, unsigned long long>((const double*)U, n_groups, N, ghost, gamma, h_max, stream);
+  return GAMER_HYDRO_INVALID_ARG;
+}
+
+int gamer_hydro_fill_ghosts(const void* U_out, void* U_in_with_ghosts, int bytes_per_real, int gx, int gy, int gz, int N,
+                            int ghost, int bc_x, int bc_y, int bc_z, cudaStream_t stream) {
+  if (bytes_per_real == 4)
+    return fill_ghosts_impl<float>((const float*)U_out, (float*)U_in_with_ghosts, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream);
+  if (bytes_per_real == 8)
+    return fill_ghosts_impl<double>((const double*)U_out, (double*)U_in_with_ghosts, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream);
+  return GAMER_HYDRO_INVALID_ARG;
+}
+
+int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, int gz, int N, int ghost, int bc_x,
+                        int bc_y, int bc_z, int n_steps, float cfl, float dx, float gamma, int limiter, float* h_dts,
+                        cudaStream_t stream) {
+  if (!U || !U_out || gx < 1 || gy < 1 || gz < 1 || n_steps < 0 || !(cfl > 0.0f) || !(dx > 0.0f))
+    return GAMER_HYDRO_INVALID_ARG;
+  const long long ng = (long long)gx * gy * gz;
+  if (ng > 0x7fffffffLL) return GAMER_HYDRO_INVALID_ARG;
+  for (int s = 0; s < n_steps; ++s) {
+    double vmax = 0.0;
+    int rc = gamer_hydro_max_speed(U, 4, (int)ng, N, ghost, (double)gamma, &vmax, stream);
+    if (rc) return rc;
+    if (!(vmax > 0.0) || vmax != vmax) return GAMER_HYDRO_INVALID_ARG;   // no finite positive signal speed: invalid input
+    const float dt = (float)((double)cfl * (double)dx / vmax);           // R15, fp64 on the host, rounded once (R11)
+    if (h_dts) h_dts[s] = dt;
+    if ((rc = gamer_hydro_step(U, U_out, bflux, (int)ng, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
+    if ((rc = gamer_hydro_fill_ghosts(U_out, U, 4, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream))) return rc;
+  }
+  return 0;
 }
 
 int gamer_hydro_step_host(const float* h_in, float* h_out, float* h_bf, int n_groups, int N, int ghost, float dt,

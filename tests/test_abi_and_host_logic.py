@@ -65,6 +65,12 @@ def test_strerror_and_argument_validation_without_a_device():
     assert L.gamer_hydro_step(None, None, None, 4, 16, 2, 1e-3, 1e-2, 5 / 3, 0, None) == 1      # null buffers
     assert L.gamer_hydro_step(None, None, None, 0, 16, 2, 1e-3, 1e-2, 5 / 3, 0, None) == 0      # empty batch: no-op
     assert L.gamer_hydro_alloc(8, 16, 2, 3, 0) == 1                                             # bytes_per_real
+    import ctypes
+    vmax = ctypes.c_double(-1.0)
+    assert L.gamer_hydro_max_speed(None, 4, 4, 16, 2, 5 / 3, ctypes.byref(vmax), None) == 1     # null array
+    assert L.gamer_hydro_max_speed(None, 2, 4, 16, 2, 5 / 3, ctypes.byref(vmax), None) == 1     # bytes_per_real
+    assert L.gamer_hydro_fill_ghosts(None, None, 4, 1, 1, 1, 16, 2, 0, 0, 0, None) == 1         # null arrays
+    assert L.gamer_hydro_advance(None, None, None, 1, 1, 1, 16, 2, 0, 0, 0, 1, 0.5, 1.0, 5 / 3, 0, None, None) == 1
 
 
 def test_no_cpu_fallback_without_a_gpu():

@@ -1,0 +1,112 @@
+"""GPU tests (-m gpu) of the steps either side of the hot path: the CFL signal-speed
+maximum (R15), the same-level ghost-shell refill (R16) and the device-resident multi-step driver. References: the
+numpy harness of paper_1007_3818_b200/workloads.py (pure data movement / the R15 formula in fp64) and, for the
+multi-step run, the fp64 oracle stepped with the time steps the device reports."""
+import numpy as np
+import pytest
+import torch
+
+import metrics
+import parity_util as pu
+import paper_1007_3818_b200 as gh
+from oracle import mhm_oracle as O
+from paper_1007_3818_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+G = wl.GAMMA
+DEV = "cuda:0"
+BC = {"periodic": gh.BC_PERIODIC, "outflow": gh.BC_OUTFLOW}
+
+
+def _grid(shape):
+    nz, ny, nx = shape
+    return (nx // 16, ny // 16, nz // 16)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+@pytest.mark.parametrize("bc", [("periodic",) * 3, ("outflow", "periodic", "outflow"), ("outflow",) * 3])
+def test_fill_ghosts_is_the_harness_ghost_fill_bit_for_bit(bc, dtype):
+    rng = np.random.default_rng(11)
+    shape = (32, 48, 64)                                    # nz, ny, nx -> 2 x 3 x 4 groups
+    U = rng.standard_normal((5,) + shape).astype(dtype)
+    want = wl.cut_groups(U, bc)                             # [G][5][20][20][20]
+    interiors = np.ascontiguousarray(want[:, :, 2:-2, 2:-2, 2:-2])
+    d_out = torch.from_numpy(interiors).to(DEV)
+    d_in = torch.full(want.shape, float("nan"), dtype=d_out.dtype, device=DEV)
+    gh.gamer_hydro_fill_ghosts(d_out, d_in, _grid(shape), bc=[BC[b] for b in bc])
+    torch.cuda.synchronize()
+    assert np.array_equal(d_in.cpu().numpy(), want)
+    # wider shell (ghost = 3) and a small patch size (N = 8)
+    want3 = wl.cut_groups(U[:, :16, :16, :24], bc, N=8, ghost=3)
+    d_out3 = torch.from_numpy(np.ascontiguousarray(want3[:, :, 3:-3, 3:-3, 3:-3])).to(DEV)
+    d_in3 = torch.empty(want3.shape, dtype=d_out.dtype, device=DEV)
+    gh.gamer_hydro_fill_ghosts(d_out3, d_in3, (3, 2, 2), N=8, ghost=3, bc=[BC[b] for b in bc])
+    torch.cuda.synchronize()
+    assert np.array_equal(d_in3.cpu().numpy(), want3)
+
+
+def test_max_speed_matches_the_fp64_formula():
+    w = wl.config_3_cosmo(64, seed=9)
+    grp = w.groups()
+    ref = wl.max_signal_speed(w.U)
+    got = gh.gamer_hydro_max_speed(torch.from_numpy(grp).to(DEV))
+    assert abs(got - ref) <= 1e-4 * ref, (got, ref)          # Mach-30 cells: P from a cancelling difference in fp32
+    got64 = gh.gamer_hydro_max_speed(torch.from_numpy(grp.astype(np.float64)).to(DEV))
+    assert abs(got64 - ref) <= 1e-12 * ref
+    # interiors without ghost shells (a U_out array), fp32 on a smooth field
+    w2 = wl.config_2_turbulence(64, seed=4)
+    inter = np.ascontiguousarray(w2.groups()[:, :, 2:-2, 2:-2, 2:-2])
+    got2 = gh.gamer_hydro_max_speed(torch.from_numpy(inter).to(DEV), ghost=0)
+    ref2 = wl.max_signal_speed(w2.U)
+    assert abs(got2 - ref2) <= 2e-6 * ref2
+    # ghost cells must not enter the maximum
+    poisoned = grp.copy()
+    poisoned[:, 1:4, :2] = 1e6
+    assert gh.gamer_hydro_max_speed(torch.from_numpy(poisoned).to(DEV)) == got
+
+
+@pytest.mark.parametrize("cfg", ["turbulence", "sod_tube"])
+def test_device_resident_advance_matches_host_driven_steps_and_the_oracle(cfg):
+    if cfg == "turbulence":
+        w, steps = wl.config_2_turbulence(64, seed=2, steps=10), 10
+    else:
+        w, steps = wl.config_1_sod_tube(nx=256, steps=10), 10
+    grid, bc = _grid(w.shape), [BC[b] for b in w.bc]
+    dx = pu.f32(w.dx)
+    d_U = torch.from_numpy(w.groups()).to(DEV)
+    n = d_U.shape[0]
+    d_out = torch.empty((n, 5, 16, 16, 16), dtype=torch.float32, device=DEV)
+    d_bf = torch.empty((n, 6, 5, 16, 16), dtype=torch.float32, device=DEV)
+    dts = gh.gamer_hydro_advance(d_U, d_out, d_bf, grid, steps, w.cfl, dx, bc=bc, limiter=w.limiter)
+    torch.cuda.synchronize()
+    assert len(dts) == steps and all(dt > 0 for dt in dts)
+    # the harness' fp64 time step on the initial box agrees with the device's first one
+    assert abs(dts[0] - wl.cfl_dt(w.U, w.dx, w.cfl)) <= 2e-6 * dts[0]
+    # (1) host-driven loop through the plain step call with the same dt sequence: bit-identical
+    U = w.U.copy()
+    for dt in dts:
+        out = pu.run_gpu(wl.cut_groups(U, w.bc), dt, dx, G, w.limiter, want_bflux=False)[0]
+        U = wl.assemble_box(out, w.shape)
+    assert np.array_equal(d_out.cpu().numpy(), out)
+    assert np.array_equal(d_U.cpu().numpy(), wl.cut_groups(U, w.bc))       # ghost shells refilled for the next step
+    # (2) the fp64 oracle with the same dt sequence: north_star's 10-step tolerance
+    Uo = w.U.astype(np.float64)
+    for dt in dts:
+        r = O.step_groups(wl.cut_groups(Uo, w.bc), 16, 2, dt, dx, G, w.limiter, want_bflux=False, want_guard=False)
+        Uo = wl.assemble_box(r.U_out, w.shape)
+    assert metrics.max_rel_err(U[None], Uo[None], G) <= 1e-3
+
+
+def test_advance_argument_errors():
+    d_U = torch.ones((1, 5, 20, 20, 20), dtype=torch.float32, device=DEV)
+    d_out = torch.empty((1, 5, 16, 16, 16), dtype=torch.float32, device=DEV)
+    with pytest.raises(gh.GamerHydroError):
+        gh.gamer_hydro_advance(d_U, d_out, None, (1, 1, 1), 1, -0.5, 1.0)           # cfl <= 0
+    with pytest.raises(gh.GamerHydroError):
+        gh.gamer_hydro_advance(d_U, d_out, None, (2, 1, 1), 1, 0.5, 1.0)            # shapes do not match the grid
+    with pytest.raises(gh.GamerHydroError):
+        gh.gamer_hydro_fill_ghosts(d_out, d_U, (1, 1, 1), bc=(0, 2, 0))             # unknown boundary code
+    d_U[:, 1:4] = 0.0
+    d_U[:, 0] = float("nan")                                                        # no finite signal speed
+    with pytest.raises(gh.GamerHydroError):
+        gh.gamer_hydro_advance(d_U, d_out, None, (1, 1, 1), 1, 0.5, 1.0)
