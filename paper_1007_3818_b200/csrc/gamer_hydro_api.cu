@@ -325,21 +325,33 @@ int max_speed_impl(const R* U, int n_groups, int N, int ghost, double gamma, dou
   return 0;
 }
 
-template <class R>
+// want_max: also accumulate the signal-speed maximum of the refilled state into the status slot (zeroed first)
+template <class R, class Bits>
 int fill_ghosts_impl(const R* U_out, R* U_in, int gx, int gy, int gz, int N, int ghost, int bcx, int bcy, int bcz,
-                     cudaStream_t stream) {
+                     cudaStream_t stream, bool want_max = false, double gamma = 5.0 / 3.0) {
   if (!U_out || !U_in || gx < 1 || gy < 1 || gz < 1 || N < 1 || ghost < 0 || (bcx | bcy | bcz) < 0 || bcx > 1 ||
       bcy > 1 || bcz > 1)
     return GAMER_HYDRO_INVALID_ARG;
+  const int S = N + 2 * ghost;
   if ((long long)gx * gy * gz > 0x7fffffffLL) return GAMER_HYDRO_INVALID_ARG;
+  if (ghost > gx * N || ghost > gy * N || ghost > gz * N) return GAMER_HYDRO_UNSUPPORTED;  // shell wider than the box
   int rc = ensure_init();
   if (rc) return rc;
-  const int S = N + 2 * ghost;
-  const long long total = (long long)gx * gy * gz * S * S * S;
-  const int threads = 256;
-  long long want = (total + threads - 1) / threads;
-  const int grid = (int)(want < (long long)g_state.sm_count * 32 ? want : (long long)g_state.sm_count * 32);
-  gh::fill_ghosts_kernel<R><<<grid, threads, 0, stream>>>(U_out, U_in, gx, gy, gz, N, ghost, bcx, bcy, bcz);
+  Bits* slot = nullptr;
+  if (want_max) {
+    slot = reinterpret_cast<Bits*>(g_state.status + 2);
+    CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
+  }
+  const int grid = gx * gy * gz;   // one CTA per group
+  if (N == 16 && ghost == 2)
+    gh::fill_ghosts_kernel<R, Bits, 2, 16, 2><<<grid, 256, 0, stream>>>(U_out, U_in, gx, gy, gz, N, ghost, bcx, bcy, bcz,
+                                                                        (R)gamma, slot);
+  else if (N % 2 == 0 && ghost % 2 == 0)
+    gh::fill_ghosts_kernel<R, Bits, 2, 0, 0><<<grid, 256, 0, stream>>>(U_out, U_in, gx, gy, gz, N, ghost, bcx, bcy, bcz,
+                                                                       (R)gamma, slot);
+  else
+    gh::fill_ghosts_kernel<R, Bits, 1, 0, 0><<<grid, 256, 0, stream>>>(U_out, U_in, gx, gy, gz, N, ghost, bcx, bcy, bcz,
+                                                                       (R)gamma, slot);
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   return 0;
@@ -405,9 +417,9 @@ int gamer_hydro_max_speed(const void* U, int bytes_per_real, int n_groups, int N
 int gamer_hydro_fill_ghosts(const void* U_out, void* U_in_with_ghosts, int bytes_per_real, int gx, int gy, int gz, int N,
                             int ghost, int bc_x, int bc_y, int bc_z, cudaStream_t stream) {
   if (bytes_per_real == 4)
-    return fill_ghosts_impl<float>((const float*)U_out, (float*)U_in_with_ghosts, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream);
+    return fill_ghosts_impl<float, unsigned int>((const float*)U_out, (float*)U_in_with_ghosts, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream);
   if (bytes_per_real == 8)
-    return fill_ghosts_impl<double>((const double*)U_out, (double*)U_in_with_ghosts, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream);
+    return fill_ghosts_impl<double, unsigned long long>((const double*)U_out, (double*)U_in_with_ghosts, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream);
   return GAMER_HYDRO_INVALID_ARG;
 }
 
@@ -418,15 +430,26 @@ int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, in
     return GAMER_HYDRO_INVALID_ARG;
   const long long ng = (long long)gx * gy * gz;
   if (ng > 0x7fffffffLL) return GAMER_HYDRO_INVALID_ARG;
+  if (n_steps == 0) return 0;
+  if (!(gamma > 1.0f)) return GAMER_HYDRO_INVALID_ARG;
+  double vmax = 0.0;
+  int rc = gamer_hydro_max_speed(U, 4, (int)ng, N, ghost, (double)gamma, &vmax, stream);   // state on entry
+  if (rc) return rc;
   for (int s = 0; s < n_steps; ++s) {
-    double vmax = 0.0;
-    int rc = gamer_hydro_max_speed(U, 4, (int)ng, N, ghost, (double)gamma, &vmax, stream);
-    if (rc) return rc;
-    if (!(vmax > 0.0) || vmax != vmax) return GAMER_HYDRO_INVALID_ARG;   // no finite positive signal speed: invalid input
-    const float dt = (float)((double)cfl * (double)dx / vmax);           // R15, fp64 on the host, rounded once (R11)
+    if (!(vmax > 0.0) || vmax > 3.0e38) return GAMER_HYDRO_INVALID_ARG;   // no finite positive signal speed: invalid state
+    const float dt = (float)((double)cfl * (double)dx / vmax);            // R15, fp64 on the host, rounded once (R11)
     if (h_dts) h_dts[s] = dt;
     if ((rc = gamer_hydro_step(U, U_out, bflux, (int)ng, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
-    if ((rc = gamer_hydro_fill_ghosts(U_out, U, 4, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream))) return rc;
+    // ghost refill fused with the signal-speed maximum of the new state (next step's dt)
+    if ((rc = fill_ghosts_impl<float, unsigned int>(U_out, U, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream, true,
+                                                    (double)gamma)))
+      return rc;
+    unsigned int bits = 0;
+    CK(cudaMemcpyAsync(&bits, g_state.status + 2, sizeof(bits), cudaMemcpyDeviceToHost, stream));
+    CK(cudaStreamSynchronize(stream));
+    float v;
+    memcpy(&v, &bits, sizeof(v));
+    vmax = (double)v;
   }
   return 0;
 }
