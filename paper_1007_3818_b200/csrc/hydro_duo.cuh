@@ -38,6 +38,18 @@ __device__ __forceinline__ void set2(f2& d, float a, float b) {
   asm volatile("mov.b64 %0, {%1, %2};" : "+l"(d.v) : "f"(a), "f"(b));
 }
 
+// Exchange arrays hold, per quantity m, FNT (lo, hi) lane pairs. GH_SPLIT_EXCH = 1 (default): the two lanes in
+// separate FNT-word planes (two 32-bit stores, conflict-free reads); 0: pair-packed (one 64-bit store per pair, but the
+// 32-bit reads of one lane are 2-way bank-conflicted). Measured on the headline configuration: 4.901 vs 4.933 ms.
+#ifndef GH_SPLIT_EXCH
+#define GH_SPLIT_EXCH 1
+#endif
+__device__ __forceinline__ int ex_off(int slot, int lane) { return GH_SPLIT_EXCH ? lane * FNT + slot : 2 * slot + lane; }
+__device__ __forceinline__ void ex_put(float* base /* + ex_off(t, 0) */, int m, f2 v) {
+  if (GH_SPLIT_EXCH) { base[m * (2 * FNT)] = lo(v); base[m * (2 * FNT) + FNT] = hi(v); }
+  else sts2(base + m * (2 * FNT), v);
+}
+
 // scalar state for the z-face solve
 struct St1 {
   float r, u, v, w, p, h;
@@ -137,7 +149,7 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
   const int vblock = (int)blockIdx.x * DHALVES + HALF, vgrid = (int)gridDim.x * DHALVES;
   auto half_sync = [&]() { asm volatile("bar.sync %0, %1;" ::"n"(1 + HALF), "n"(FNT) : "memory"); };
   float* const wring = reinterpret_cast<float*>(smem + SM::off_w);
-  float* const stx = reinterpret_cast<float*>(smem + SM::off_st);   // pairs: [buf][m][t][lane]
+  float* const stx = reinterpret_cast<float*>(smem + SM::off_st);   // [buf][m][ex_off(t, lane)]
   float* const flx = reinterpret_cast<float*>(smem + SM::off_fl);
   const uint32_t raw_base = smem_u32(smem + SM::off_raw);
   const uint32_t bar_base = smem_u32(smem + SM::off_bar);
@@ -329,9 +341,9 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
         {
           const St2 SB = state_from_face(WB, dUrot, c, gmin);
           if (!ghost_plane) {
-            float* so = stx + (buf * (6 * FNT) + t) * 2;
-            sts2(so + 0 * (2 * FNT), SB.r); sts2(so + 1 * (2 * FNT), SB.u); sts2(so + 2 * (2 * FNT), SB.v);
-            sts2(so + 3 * (2 * FNT), SB.w); sts2(so + 4 * (2 * FNT), SB.p); sts2(so + 5 * (2 * FNT), SB.h);
+            float* so = stx + buf * (12 * FNT) + ex_off(t, 0);
+            ex_put(so, 0, SB.r); ex_put(so, 1, SB.u); ex_put(so, 2, SB.v);
+            ex_put(so, 3, SB.w); ex_put(so, 4, SB.p); ex_put(so, 5, SB.h);
           }
         }
         SA = state_from_face(WA, dUrot, c, gmin);
@@ -347,9 +359,9 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
           set2(SC.r, Wc[0], Wc[0]); set2(SC.u, Wc[1], Wc[2]); set2(SC.v, Wc[2], Wc[1]); set2(SC.w, Wc[3], Wc[3]);
           set2(SC.p, Wc[4], Wc[4]); set2(SC.h, h, h);
           if (!ghost_plane) {
-            float* so = stx + (buf * (6 * FNT) + t) * 2;
-            sts2(so + 0 * (2 * FNT), SA.r); sts2(so + 1 * (2 * FNT), SA.u); sts2(so + 2 * (2 * FNT), SA.v);
-            sts2(so + 3 * (2 * FNT), SA.w); sts2(so + 4 * (2 * FNT), SA.p); sts2(so + 5 * (2 * FNT), SA.h);
+            float* so = stx + buf * (12 * FNT) + ex_off(t, 0);
+            ex_put(so, 0, SA.r); ex_put(so, 1, SA.u); ex_put(so, 2, SA.v);
+            ex_put(so, 3, SA.w); ex_put(so, 4, SA.p); ex_put(so, 5, SA.h);
           }
           n_guard += 1u;  // every cell that gets here is one whose states are used
         }
@@ -378,8 +390,8 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
       flux_wait();  // x / y fluxes of plane k-1 visible (published before the END of the previous plane)
       // ---- E: conservative update of plane k-1 (its x / y fluxes were published one phase earlier)
       if (interior && k >= 1) {
-        const float* fxb = flx + ((buf ^ 1) * (5 * FNT) + t) * 2 + 2;      // lane lo: Fx of the upper x neighbour
-        const float* fyb = flx + ((buf ^ 1) * (5 * FNT) + t_yu) * 2 + 1;  // lane hi: Fy (slot order) of the upper y neighbour
+        const float* fxb = flx + (buf ^ 1) * (10 * FNT) + ex_off(t + 1, 0);  // lane lo: Fx of the upper x neighbour
+        const float* fyb = flx + (buf ^ 1) * (10 * FNT) + ex_off(t_yu, 1);   // lane hi: Fy (slot order) of the upper y neighbour
         const int us = (int)rs - 3 + ((int)rs < 3 ? DNSTAGE : 0);  // slot of plane k-1 (rs points at plane k+2)
         const float* rawp = reinterpret_cast<const float*>(smem + SM::off_raw + us * SM::raw_stage_bytes) + raw_own;
         float* op = outg + (k - 1) * (FN * FN) + j * FN + i;
@@ -398,8 +410,8 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
 
       // ---- D: Roe fluxes at the lower x face (lane x) and the lower y face (lane y) of plane k, one packed solve
       if (!ghost_plane) {
-        const float* xl = stx + (buf * (6 * FNT) + t) * 2 - 2;      // lane lo of the lower x neighbour's pair
-        const float* yl = stx + (buf * (6 * FNT) + t_yl) * 2 + 1;  // lane hi of the lower y neighbour's pair
+        const float* xl = stx + buf * (12 * FNT) + ex_off(t - 1, 0);  // lane lo of the lower x neighbour's pair
+        const float* yl = stx + buf * (12 * FNT) + ex_off(t_yl, 1);   // lane hi of the lower y neighbour's pair
         St2 L;
         L.r = mk2(xl[0 * (2 * FNT)], yl[0 * (2 * FNT)]); L.u = mk2(xl[1 * (2 * FNT)], yl[1 * (2 * FNT)]);
         L.v = mk2(xl[2 * (2 * FNT)], yl[2 * (2 * FNT)]); L.w = mk2(xl[3 * (2 * FNT)], yl[3 * (2 * FNT)]);
@@ -408,10 +420,10 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
         roe2<0>(L, SA, c, F);
         // lane x is in global component order; lane y comes back as (rho, my, mx, mz, E)
         const float Fy[5] = {hi(F[0]), hi(F[2]), hi(F[1]), hi(F[3]), hi(F[4])};
-        float* fo = flx + (buf * (5 * FNT) + t) * 2;
+        float* fo = flx + buf * (10 * FNT) + ex_off(t, 0);
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
-          sts2(fo + q * (2 * FNT), F[q]);
+          ex_put(fo, q, F[q]);
           accd[q] = (lo(F[q]) + Fy[q]) + Fz[q];  // sum of the lower-face fluxes of plane k
         }
         if (bfg) {  // a5: outer faces of this plane
