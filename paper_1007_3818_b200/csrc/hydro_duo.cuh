@@ -1,13 +1,16 @@
 // csrc/hydro_duo.cuh — fp32 performance path, variant "duo": ONE cell per thread (the 320-thread cross of
-// hydro_fused.cuh, 96 registers, two CTAs = 20 warps per SM) but with the two LANES of every Blackwell `*.f32x2`
-// instruction carrying two directions of the same cell instead of two cells:
+// hydro_fused.cuh, 96 registers, 20 warps per SM) with the two LANES of every Blackwell `*.f32x2` instruction
+// carrying two directions of the same cell instead of two cells:
 //   lanes (x, y)  for the '+' face states, the '-' face states, their own-direction fluxes and the x / y Roe solves
 //                 (the y lane holds its velocity components as (v, u, w) so that slot 1 is the normal one),
 //   lanes (z-, z+) for the two z face states and their fluxes (same slot orders, slot 3 = w is normal in both).
 // The packed forms keep the issue-slot saving of hydro_pair.cuh (half the slots per FLOP) without its register
 // appetite, so five warps per scheduler stay resident to hide the dependent-issue latency (profiles/r1c_README.md).
-// Schedule per plane as in hydro_pair.cuh: ONE split (arrive / wait) CTA barrier, everything a neighbour publishes is
-// double-buffered and consumed one phase later. Follows PAPER.md:15 with the readings of DESIGN.md §3.
+// Schedule per plane: TWO split (arrive / wait) mbarrier barriers — "states of plane k published" and "x / y fluxes of
+// plane k published" — instead of __syncthreads; everything a neighbour publishes is double-buffered and consumed one
+// phase later, and the work between an arrive and its wait absorbs the skew between warps.
+// One CTA = two independent 320-thread halves (own shared-memory region, TMA ring and barriers), so that the 20 warps
+// of an SM sit five on each scheduler (profiles/r1d_README.md). Follows PAPER.md:15 with the readings of DESIGN.md §3.
 #pragma once
 #include <cuda.h>
 #include <stdint.h>
