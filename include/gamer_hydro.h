@@ -106,12 +106,23 @@ int gamer_hydro_max_speed(const void* U, int bytes_per_real, int n_groups, int N
 int gamer_hydro_fill_ghosts(const void* U_out, void* U_in_with_ghosts, int bytes_per_real, int gx, int gy, int gz, int N,
                             int ghost, int bc_x, int bc_y, int bc_z, cudaStream_t stream);
 
+/* One fp32 step of a FULLY PERIODIC uniform grid with the halo exchange fused into the step kernel: besides U_out
+ * and boundary_fluxes (as gamer_hydro_step) the kernel writes every updated cell straight into
+ * U_next_with_ghosts [G][5][20][20][20] — its own interior position and the ghost shells of the up to seven
+ * neighbouring groups it borders — so that U_next is the complete ghosted input of the next step (bit-identical to
+ * gamer_hydro_fill_ghosts applied to U_out), and accumulates the signal-speed maximum of the new state for
+ * gamer_hydro_advance. N = 16, ghost = 2 only (else GAMER_HYDRO_UNSUPPORTED); U_next must not alias U. */
+int gamer_hydro_step_grid(const float* U_with_ghosts, float* U_out, float* boundary_fluxes, float* U_next_with_ghosts,
+                          int gx, int gy, int gz, int N, int ghost, float dt, float dx, float gamma, int limiter,
+                          cudaStream_t stream);
+
 /* n_steps time steps of the fp32 path on one uniform grid without leaving the device: per step
  * dt = float(cfl * dx / max signal speed) (fp64 on the host from the device-side maximum, R15/R11), then
  * gamer_hydro_step, then gamer_hydro_fill_ghosts. U (ghost shells filled on entry) holds the final state with
  * refilled ghost shells on return, U_out the interiors of the last step, boundary_fluxes (may be NULL) those of
  * the last step; h_dts (HOST, n_steps floats, may be NULL) receives the time steps taken. One 4-byte
- * device-to-host read and one stream synchronisation per step. */
+ * device-to-host read and one stream synchronisation per step. On a fully periodic grid of 16^3 groups the loop uses
+ * gamer_hydro_step_grid, ping-ponging between U and a second ghosted array the library allocates (and keeps). */
 int gamer_hydro_advance(float* U_with_ghosts, float* U_out, float* boundary_fluxes, int gx, int gy, int gz, int N,
                         int ghost, int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dx, float gamma,
                         int limiter, float* h_dts, cudaStream_t stream);

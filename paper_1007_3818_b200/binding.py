@@ -19,7 +19,8 @@ PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_PAIR = 0, 1, 
 
 EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
-           "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance"]
+           "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance",
+           "gamer_hydro_step_grid"]
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
@@ -45,6 +46,7 @@ def lib():
         L.gamer_hydro_set_path.argtypes = [i]
         L.gamer_hydro_max_speed.argtypes = [vp, i, i, i, i, d, C.POINTER(C.c_double), vp]
         L.gamer_hydro_fill_ghosts.argtypes = [vp, vp, i, i, i, i, i, i, i, i, i, vp]
+        L.gamer_hydro_step_grid.argtypes = [vp, vp, vp, vp, i, i, i, i, i, f, f, f, i, vp]
         L.gamer_hydro_advance.argtypes = [vp, vp, vp, i, i, i, i, i, i, i, i, i, f, f, f, i, vp, vp]
         L.gamer_hydro_launch_count.restype = C.c_ulonglong
         L.gamer_hydro_strerror.restype = C.c_char_p
@@ -151,6 +153,23 @@ def gamer_hydro_fill_ghosts(U_out, U_in_with_ghosts, grid, N=16, ghost=2, bc=(BC
     _check(lib().gamer_hydro_fill_ghosts(U_out.data_ptr(), U_in_with_ghosts.data_ptr(), _real_bytes(U_out), gx, gy, gz,
                                          N, ghost, int(bc[0]), int(bc[1]), int(bc[2]), _stream_ptr(stream)))
     return U_in_with_ghosts
+
+
+def gamer_hydro_step_grid(U_with_ghosts, U_out, boundary_fluxes, U_next_with_ghosts, grid, dt, dx, N=16, ghost=2,
+                          gamma=5.0 / 3.0, limiter=MINMOD, stream=None):
+    """One fp32 step of a fully periodic uniform grid; the kernel also writes the next step's ghosted array."""
+    gx, gy, gz = (int(v) for v in grid)
+    G, S = gx * gy * gz, N + 2 * ghost
+    if tuple(U_with_ghosts.shape) != (G, 5, S, S, S) or tuple(U_next_with_ghosts.shape) != (G, 5, S, S, S) or \
+            tuple(U_out.shape) != (G, 5, N, N, N):
+        raise GamerHydroError("shapes do not match a %dx%dx%d grid of groups" % (gx, gy, gz))
+    for x in (U_with_ghosts, U_out, boundary_fluxes, U_next_with_ghosts):
+        if x is not None and not (x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()):
+            raise GamerHydroError("tensors must be contiguous CUDA float32 tensors")
+    bf = boundary_fluxes.data_ptr() if boundary_fluxes is not None else None
+    _check(lib().gamer_hydro_step_grid(U_with_ghosts.data_ptr(), U_out.data_ptr(), bf, U_next_with_ghosts.data_ptr(),
+                                       gx, gy, gz, N, ghost, dt, dx, gamma, int(limiter), _stream_ptr(stream)))
+    return U_next_with_ghosts
 
 
 def gamer_hydro_advance(U_with_ghosts, U_out, boundary_fluxes, grid, n_steps, cfl, dx, N=16, ghost=2,

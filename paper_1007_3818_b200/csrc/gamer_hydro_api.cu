@@ -38,6 +38,8 @@ struct State {
   void* hbuf_bf[3] = {nullptr, nullptr, nullptr};
   size_t hbuf_groups = 0;
   int hbuf_N = 0, hbuf_ghost = 0;
+  void* grid_buf = nullptr;              // gamer_hydro_advance: second ghosted array for the fused-halo ping-pong
+  size_t grid_buf_bytes = 0;
   int path = GAMER_HYDRO_PATH_AUTO;
   char cuda_msg[256] = "no CUDA error recorded";
   EncodeTiledFn encode = nullptr;
@@ -90,6 +92,8 @@ int init_locked(int device) {
   CK(cudaFuncSetAttribute(gh::pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
   CK(cudaFuncSetAttribute(gh::duo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
+  CK(cudaFuncSetAttribute(gh::duo_halo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
+  CK(cudaFuncSetAttribute(gh::duo_halo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
@@ -198,7 +202,7 @@ int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int gho
 
 // fp32 performance path: one cell per thread, the f32x2 lanes carry two directions of the cell (hydro_duo.cuh)
 int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
-               float gamma, int limiter, cudaStream_t stream) {
+               float gamma, int limiter, cudaStream_t stream, const gh::HaloGrid* halo = nullptr) {
   CUtensorMap map;
   int rc = encode_plane_map<float>(U_in, n_groups, N, ghost, map);
   if (rc) return rc;
@@ -206,10 +210,17 @@ int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int 
   const int smem = gh::DHALVES * gh::DuoSmem::total_padded;   // one CTA per SM: two independent 320-thread halves
   const int want = (n_groups + gh::DHALVES - 1) / gh::DHALVES;
   const int grid = want < g_state.sm_count ? want : g_state.sm_count;
-  if (limiter == 0)
-    gh::duo_kernel<0><<<grid, gh::FNT * gh::DHALVES, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
-  else
-    gh::duo_kernel<1><<<grid, gh::FNT * gh::DHALVES, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  const int threads = gh::FNT * gh::DHALVES;
+  if (halo) {
+    if (limiter == 0)
+      gh::duo_halo_kernel<0><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status, *halo);
+    else
+      gh::duo_halo_kernel<1><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status, *halo);
+  } else if (limiter == 0) {
+    gh::duo_kernel<0><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  } else {
+    gh::duo_kernel<1><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  }
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   return 0;
@@ -387,6 +398,9 @@ void gamer_hydro_free(void) {
   for (int s = 0; s < 3; ++s)
     if (g_state.hstream[s]) { cudaStreamDestroy(g_state.hstream[s]); g_state.hstream[s] = nullptr; }
   if (g_state.scratch) cudaFree(g_state.scratch);
+  if (g_state.grid_buf) cudaFree(g_state.grid_buf);
+  g_state.grid_buf = nullptr;
+  g_state.grid_buf_bytes = 0;
   if (g_state.status) cudaFree(g_state.status);
   g_state.scratch = nullptr;
   g_state.scratch_bytes = 0;
@@ -423,6 +437,21 @@ int gamer_hydro_fill_ghosts(const void* U_out, void* U_in_with_ghosts, int bytes
   return GAMER_HYDRO_INVALID_ARG;
 }
 
+int gamer_hydro_step_grid(const float* U, float* U_out, float* bflux, float* U_next, int gx, int gy, int gz, int N,
+                          int ghost, float dt, float dx, float gamma, int limiter, cudaStream_t stream) {
+  if (gx < 1 || gy < 1 || gz < 1 || (long long)gx * gy * gz > 0x7fffffffLL || !U_next || U_next == U)
+    return GAMER_HYDRO_INVALID_ARG;
+  const int ng = gx * gy * gz;
+  int rc = validate<float>(U, U_out, bflux, ng, N, ghost, dt, dx, gamma, limiter);
+  if (rc) return rc;
+  if (N != gh::FN || ghost != 2) return GAMER_HYDRO_UNSUPPORTED;   // the fused-halo kernel is the N = 16, ghost = 2 one
+  if ((rc = ensure_init())) return rc;
+  unsigned int* slot = reinterpret_cast<unsigned int*>(g_state.status + 2);
+  CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
+  const gh::HaloGrid hg = {U_next, slot, gx, gy, gz};
+  return launch_duo(U, U_out, bflux, ng, N, ghost, dt, dx, gamma, limiter, stream, &hg);
+}
+
 int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, int gz, int N, int ghost, int bc_x,
                         int bc_y, int bc_z, int n_steps, float cfl, float dx, float gamma, int limiter, float* h_dts,
                         cudaStream_t stream) {
@@ -431,25 +460,53 @@ int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, in
   const long long ng = (long long)gx * gy * gz;
   if (ng > 0x7fffffffLL) return GAMER_HYDRO_INVALID_ARG;
   if (n_steps == 0) return 0;
-  if (!(gamma > 1.0f)) return GAMER_HYDRO_INVALID_ARG;
+  if (!(gamma > 1.0f) || N < 1 || ghost < 2) return GAMER_HYDRO_INVALID_ARG;
   double vmax = 0.0;
   int rc = gamer_hydro_max_speed(U, 4, (int)ng, N, ghost, (double)gamma, &vmax, stream);   // state on entry
   if (rc) return rc;
+  // Fully periodic grid of 16^3 groups on the default path: the step kernel itself writes the next step's ghosted
+  // array and signal-speed maximum (ping-pong between U and a library-owned second array). Otherwise: step + refill.
+  const bool fused_halo = bc_x == 0 && bc_y == 0 && bc_z == 0 && N == gh::FN && ghost == 2 &&
+                          (g_state.path == GAMER_HYDRO_PATH_AUTO || g_state.path == GAMER_HYDRO_PATH_FUSED);
+  float* cur = U;
+  float* nxt = nullptr;
+  if (fused_halo) {
+    const size_t bytes = (size_t)ng * 5 * 20 * 20 * 20 * sizeof(float);
+    std::lock_guard<std::mutex> lk(g_mutex);
+    if (g_state.grid_buf_bytes < bytes) {
+      CK(cudaDeviceSynchronize());
+      if (g_state.grid_buf) cudaFree(g_state.grid_buf);
+      g_state.grid_buf = nullptr;
+      g_state.grid_buf_bytes = 0;
+      CK(cudaMalloc(&g_state.grid_buf, bytes));
+      g_state.grid_buf_bytes = bytes;
+    }
+    nxt = (float*)g_state.grid_buf;
+  }
   for (int s = 0; s < n_steps; ++s) {
     if (!(vmax > 0.0) || vmax > 3.0e38) return GAMER_HYDRO_INVALID_ARG;   // no finite positive signal speed: invalid state
     const float dt = (float)((double)cfl * (double)dx / vmax);            // R15, fp64 on the host, rounded once (R11)
     if (h_dts) h_dts[s] = dt;
-    if ((rc = gamer_hydro_step(U, U_out, bflux, (int)ng, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
-    // ghost refill fused with the signal-speed maximum of the new state (next step's dt)
-    if ((rc = fill_ghosts_impl<float, unsigned int>(U_out, U, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream, true,
-                                                    (double)gamma)))
-      return rc;
+    if (fused_halo) {
+      if ((rc = gamer_hydro_step_grid(cur, U_out, bflux, nxt, gx, gy, gz, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
+      float* tmp = cur; cur = nxt; nxt = tmp;
+    } else {
+      if ((rc = gamer_hydro_step(U, U_out, bflux, (int)ng, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
+      // ghost refill fused with the signal-speed maximum of the new state (next step's dt)
+      if ((rc = fill_ghosts_impl<float, unsigned int>(U_out, U, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream, true,
+                                                      (double)gamma)))
+        return rc;
+    }
     unsigned int bits = 0;
     CK(cudaMemcpyAsync(&bits, g_state.status + 2, sizeof(bits), cudaMemcpyDeviceToHost, stream));
     CK(cudaStreamSynchronize(stream));
     float v;
     memcpy(&v, &bits, sizeof(v));
     vmax = (double)v;
+  }
+  if (cur != U) {  // odd number of fused steps: the final state sits in the library's array
+    CK(cudaMemcpyAsync(U, cur, (size_t)ng * 5 * 20 * 20 * 20 * sizeof(float), cudaMemcpyDeviceToDevice, stream));
+    CK(cudaStreamSynchronize(stream));
   }
   return 0;
 }

@@ -32,7 +32,8 @@ struct DuoSmem {
   static constexpr int off_fl = off_st + 2 * 6 * FNT * 8;           // 2 x 5 x FNT x (Fx, Fy in slot order) at the lower faces
   static constexpr int off_bar = ((off_fl + 2 * 5 * FNT * 8 + 15) / 16) * 16;
   static constexpr int off_sync = off_bar + DNSTAGE * 8;
-  static constexpr int total = off_sync + 16;
+  static constexpr int off_nbr = off_sync + 16;                // HALO: 2 x 27 neighbour group ids (+ pad)
+  static constexpr int total = off_nbr + 2 * 32 * 4;
   static constexpr int total_padded = ((total + 127) / 128) * 128;   // one half-CTA's region
 };
 
@@ -137,10 +138,21 @@ __device__ __forceinline__ float limited_slope1(float a, float b) {
 
 // One half-CTA (320 threads). HALF is a template parameter so that every shared-memory address and the named
 // barrier id stay compile-time constants: a run-time half offset costs registers this kernel does not have.
-template <int LIM, int HALF>
+// Grid description of the fused-halo variant (HALO = true): the batch is ONE periodic uniform grid of gx x gy x gz
+// groups (x-fastest index); besides U_out the kernel writes every updated cell straight into the ghosted array of the
+// NEXT step — its own interior position and the ghost shells of up to seven neighbouring groups — and accumulates the
+// signal-speed maximum of the new state, so that a multi-step run needs no separate ghost-refill pass.
+struct HaloGrid {
+  float* U_next;        // [G][5][20][20][20], must not alias the input
+  unsigned int* vmax;   // bit pattern of the running maximum (zeroed by the caller)
+  int gx, gy, gz;
+};
+
+template <int LIM, int HALF, bool HALO>
 __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __restrict__ U_out, float* __restrict__ bflux,
                                          int n_groups, int goff, const PairConst& c,
-                                         unsigned long long* __restrict__ status, unsigned char* smem_cta) {
+                                         unsigned long long* __restrict__ status, unsigned char* smem_cta,
+                                         const HaloGrid& hg) {
   using SM = DuoSmem;
   // The CTA is TWO independent halves of 320 threads (10 warps), each with its own shared-memory region, group
   // stream, TMA ring and barriers. Why one 20-warp CTA instead of two 10-warp CTAs: a 10-warp CTA puts 3, 3, 2, 2
@@ -235,9 +247,17 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
   };
 
   unsigned int n_guard = 0, n_nonpos = 0;
+  float vmax_thread = 0.0f;                                   // HALO only
+  int* const nbr_tab = reinterpret_cast<int*>(smem + SM::off_nbr);
 
   for (int it = 0; it < n_local; ++it) {
     const int g = vblock + it * vgrid;
+    if (HALO && t < 27) {  // neighbour group ids of this group (periodic), double-buffered by group parity
+      const int bx = g % hg.gx, by = (g / hg.gx) % hg.gy, bz = g / (hg.gx * hg.gy);
+      const int ox = t % 3 - 1, oy = (t / 3) % 3 - 1, oz = t / 9 - 1;
+      const int nx_ = (bx + ox + hg.gx) % hg.gx, ny_ = (by + oy + hg.gy) % hg.gy, nz_ = (bz + oz + hg.gz) % hg.gz;
+      nbr_tab[(it & 1) * 32 + t] = (nz_ * hg.gy + ny_) * hg.gx + nx_;
+    }
     const int seq0 = it * FPLANES;
     float* const outg = U_out + (size_t)g * (5 * FN * FN * FN);
     float* const bfg = bflux ? bflux + (size_t)g * (30 * FN * FN) : nullptr;
@@ -407,6 +427,38 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
         }
         const float m2 = fmaf(out[3], out[3], fmaf(out[2], out[2], out[1] * out[1]));
         n_nonpos += (out[0] > 0.0f && (out[0] + out[0]) * out[4] > m2) ? 0u : 1u;
+        if (HALO) {
+          // signal speed of the new state (R15) for the next time step
+          const float ir = rcp1(out[0]);
+          const float P = fmaxf(lo(c.g1) * fmaf(-0.5f * m2, ir, out[4]), 0.0f);
+          const float sp = (fabsf(out[1]) + fabsf(out[2]) + fabsf(out[3])) * ir + 3.0f * sqrt1((lo(c.g1) + 1.0f) * P * ir);
+          vmax_thread = sp > vmax_thread ? sp : vmax_thread;
+          // the cell in the next step's ghosted array: own interior position, and the ghost shells of the neighbours
+          // it is within two cells of (per axis: none, or the one at -1 / +1)
+          const int kk = k - 1;
+          const int sx = i < 2 ? -1 : (i >= FN - 2 ? 1 : 0), sy = j < 2 ? -1 : (j >= FN - 2 ? 1 : 0);
+          const int sz = kk < 2 ? -1 : (kk >= FN - 2 ? 1 : 0);
+          const int* nt = nbr_tab + (it & 1) * 32;
+#pragma unroll
+          for (int oz = 0; oz < 2; ++oz) {
+            if (oz && !sz) continue;
+            const int zc = oz ? kk + 2 - FN * sz : kk + 2;
+#pragma unroll
+            for (int oy = 0; oy < 2; ++oy) {
+              if (oy && !sy) continue;
+              const int yc = oy ? j + 2 - FN * sy : j + 2;
+#pragma unroll
+              for (int ox = 0; ox < 2; ++ox) {
+                if (ox && !sx) continue;
+                const int xc = ox ? i + 2 - FN * sx : i + 2;
+                const int gid = nt[(oz * sz + 1) * 9 + (oy * sy + 1) * 3 + (ox * sx + 1)];
+                float* np_ = hg.U_next + (size_t)gid * (5 * FS * FS * FS) + (zc * FS + yc) * FS + xc;
+#pragma unroll
+                for (int q = 0; q < 5; ++q) np_[q * (FS * FS * FS)] = out[q];
+              }
+            }
+          }
+        }
       }
       cta_wait();  // x+ / y+ states of plane k and primitives of plane k+1 visible
       if (t == 0) issue_upto(seq0 + k + 1 + DNSTAGE);
@@ -453,6 +505,13 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
     if (n_guard) atomicAdd(&status[0], (unsigned long long)n_guard);
     if (n_nonpos) atomicAdd(&status[1], (unsigned long long)n_nonpos);
   }
+  if (HALO) {
+    for (int o = 16; o > 0; o >>= 1) {
+      const float other = __shfl_xor_sync(0xffffffffu, vmax_thread, o);
+      vmax_thread = other > vmax_thread ? other : vmax_thread;
+    }
+    if ((t & 31) == 0) atomicMax(hg.vmax, __float_as_uint(vmax_thread));
+  }
 }
 
 template <int LIM>
@@ -460,8 +519,20 @@ __global__ void __launch_bounds__(FNT * DHALVES, 1)
     duo_kernel(const __grid_constant__ CUtensorMap in_map, float* __restrict__ U_out, float* __restrict__ bflux,
                int n_groups, int goff, const __grid_constant__ PairConst c, unsigned long long* __restrict__ status) {
   extern __shared__ __align__(128) unsigned char smem_cta[];
-  if (threadIdx.x < FNT) duo_half<LIM, 0>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta);
-  else duo_half<LIM, 1>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta);
+  const HaloGrid none = {nullptr, nullptr, 1, 1, 1};
+  if (threadIdx.x < FNT) duo_half<LIM, 0, false>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta, none);
+  else duo_half<LIM, 1, false>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta, none);
+}
+
+// the fused-halo variant: same step, plus the next step's ghosted array and signal-speed maximum (HaloGrid)
+template <int LIM>
+__global__ void __launch_bounds__(FNT * DHALVES, 1)
+    duo_halo_kernel(const __grid_constant__ CUtensorMap in_map, float* __restrict__ U_out, float* __restrict__ bflux,
+                    int n_groups, int goff, const __grid_constant__ PairConst c, unsigned long long* __restrict__ status,
+                    const __grid_constant__ HaloGrid hg) {
+  extern __shared__ __align__(128) unsigned char smem_cta[];
+  if (threadIdx.x < FNT) duo_half<LIM, 0, true>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta, hg);
+  else duo_half<LIM, 1, true>(in_map, U_out, bflux, n_groups, goff, c, status, smem_cta, hg);
 }
 
 }  // namespace gh

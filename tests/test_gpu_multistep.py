@@ -110,3 +110,62 @@ def test_advance_argument_errors():
     d_U[:, 0] = float("nan")                                                        # no finite signal speed
     with pytest.raises(gh.GamerHydroError):
         gh.gamer_hydro_advance(d_U, d_out, None, (1, 1, 1), 1, 0.5, 1.0)
+
+
+@pytest.mark.parametrize("shape,limiter", [((16, 16, 16), 0), ((16, 32, 48), 1), ((64, 64, 64), 0)])
+def test_fused_halo_step_equals_step_plus_ghost_refill(shape, limiter):
+    """gamer_hydro_step_grid: the step kernel that writes the next step's ghosted array itself gives the same bits as
+    gamer_hydro_step followed by gamer_hydro_fill_ghosts — also on grids of one or two groups per axis, where a group
+    is its own periodic neighbour — and the same U_out / boundary fluxes."""
+    rng = np.random.default_rng(5)
+    nz, ny, nx = shape
+    rho = np.exp(0.3 * rng.standard_normal(shape))
+    v = 0.4 * rng.standard_normal((3,) + shape)
+    P = np.exp(0.2 * rng.standard_normal(shape))
+    U = wl.prim_box_to_cons(rho, v[0], v[1], v[2], P).astype(np.float32)
+    bc = ("periodic",) * 3
+    grid = _grid(shape)
+    grp = wl.cut_groups(U, bc)
+    n = grp.shape[0]
+    dx = pu.f32(1.0 / nx)
+    dt = wl.cfl_dt(U, 1.0 / nx, 0.4)
+    d_in = torch.from_numpy(np.array(grp)).to(DEV)
+    outs = []
+    for fused in (False, True):
+        d_out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float32, device=DEV)
+        d_bf = torch.full((n, 6, 5, 16, 16), float("nan"), dtype=torch.float32, device=DEV)
+        d_next = torch.full(grp.shape, float("nan"), dtype=torch.float32, device=DEV)
+        if fused:
+            gh.gamer_hydro_step_grid(d_in, d_out, d_bf, d_next, grid, dt, dx, limiter=limiter)
+        else:
+            gh.gamer_hydro_step(d_in, d_out, d_bf, n, 16, 2, dt, dx, G, limiter)
+            gh.gamer_hydro_fill_ghosts(d_out, d_next, grid)
+        torch.cuda.synchronize()
+        outs.append((d_out.cpu().numpy(), d_bf.cpu().numpy(), d_next.cpu().numpy()))
+    for a, b in zip(outs[0], outs[1]):
+        assert np.isfinite(b).all()
+        assert np.array_equal(a, b)
+    # and the next ghosted array is what the harness builds from the interiors
+    assert np.array_equal(outs[1][2], wl.cut_groups(wl.assemble_box(outs[1][0], shape), bc))
+    with pytest.raises(gh.GamerHydroError):
+        gh.gamer_hydro_step_grid(d_in, d_out, d_bf, d_in, grid, dt, dx)        # U_next aliases the input
+
+
+def test_advance_odd_and_even_step_counts_on_a_periodic_grid():
+    """The fused-halo loop ping-pongs between the caller's array and the library's: the caller's array must hold the
+    final ghosted state for odd and even step counts alike."""
+    w = wl.config_2_turbulence(32, seed=7)
+    grid, bc = _grid(w.shape), [BC[b] for b in w.bc]
+    dx = pu.f32(w.dx)
+    for steps in (1, 2, 3):
+        d_U = torch.from_numpy(w.groups()).to(DEV)
+        n = d_U.shape[0]
+        d_out = torch.empty((n, 5, 16, 16, 16), dtype=torch.float32, device=DEV)
+        dts = gh.gamer_hydro_advance(d_U, d_out, None, grid, steps, w.cfl, dx, bc=bc, limiter=w.limiter)
+        torch.cuda.synchronize()
+        U = w.U.copy()
+        for dt in dts:
+            out = pu.run_gpu(wl.cut_groups(U, w.bc), dt, dx, G, w.limiter, want_bflux=False)[0]
+            U = wl.assemble_box(out, w.shape)
+        assert np.array_equal(d_out.cpu().numpy(), out)
+        assert np.array_equal(d_U.cpu().numpy(), wl.cut_groups(U, w.bc)), steps
