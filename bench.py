@@ -255,7 +255,7 @@ def main():
     hbm_gbs = BYTES_PER_CELL * cells / (ms_launch * 1e-3) / 1e9
     traffic = None
     try:
-        with open(os.path.join(ROOT, "profiles", "traffic_bytes_per_launch.json")) as f:
+        with open(os.path.join(ROOT, "profiles", "r1d_traffic_bytes_per_launch.txt")) as f:
             tj = json.load(f)
             if tj.get("n_groups") == G:
                 traffic = tj["dram_bytes_read_plus_write"]
