@@ -343,7 +343,6 @@ int fill_ghosts_impl(const R* U_out, R* U_in, int gx, int gy, int gz, int N, int
   if (!U_out || !U_in || gx < 1 || gy < 1 || gz < 1 || N < 1 || ghost < 0 || (bcx | bcy | bcz) < 0 || bcx > 1 ||
       bcy > 1 || bcz > 1)
     return GAMER_HYDRO_INVALID_ARG;
-  const int S = N + 2 * ghost;
   if ((long long)gx * gy * gz > 0x7fffffffLL) return GAMER_HYDRO_INVALID_ARG;
   if (ghost > gx * N || ghost > gy * N || ghost > gz * N) return GAMER_HYDRO_UNSUPPORTED;  // shell wider than the box
   int rc = ensure_init();

@@ -41,13 +41,13 @@ __device__ __forceinline__ f2 mk2(float a, float b) {
   return r;
 }
 __device__ __forceinline__ float lo(f2 a) {
-  float x, y;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(a.v));
+  float x;
+  asm("mov.b64 {%0, _}, %1;" : "=f"(x) : "l"(a.v));
   return x;
 }
 __device__ __forceinline__ float hi(f2 a) {
-  float x, y;
-  asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(a.v));
+  float y;
+  asm("mov.b64 {_, %0}, %1;" : "=f"(y) : "l"(a.v));
   return y;
 }
 __device__ __forceinline__ f2 splat(float c) { return mk2(c, c); }
