@@ -111,7 +111,7 @@ def run_reference(args, rank, world):
     if rank != 0:
         return
     from oracle import mhm_oracle as O
-    w, groups, dt, dx, _ = make_workload(64, args.seed)      # 64 groups of the same recipe: a bounded sample
+    w, groups, dt, dx, _ = make_workload(128, args.seed)     # 512 groups of the same recipe: a bounded sample
     sample = groups[: args.ref_groups]
     for _ in range(args.warmup):
         O.step_groups(sample, N, GHOST, dt, dx, w.gamma, w.limiter, want_guard=False)
@@ -121,7 +121,7 @@ def run_reference(args, rank, world):
     t = time.perf_counter() - t0
     cells = sample.shape[0] * N ** 3 * args.steps
     val = cells / t
-    desc = "%d groups of the cfg3 recipe (64^3 box) per step, all host cores" % sample.shape[0]
+    desc = "%d groups of the cfg3 recipe (128^3 box) per step, all host cores" % sample.shape[0]
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps,
@@ -142,8 +142,9 @@ def main():
     ap.add_argument("--box", type=int, default=512, help="global box edge; 512 -> 32768 groups (headline)")
     ap.add_argument("--seed", type=int, default=3)
     ap.add_argument("--e2e-steps", type=int, default=3)
-    ap.add_argument("--cpu-groups", type=int, default=192, help="groups in the oracle sample (cpu_baseline)")
-    ap.add_argument("--ref-groups", type=int, default=64)
+    ap.add_argument("--cpu-groups", type=int, default=4096,
+                    help="groups in the oracle sample (cpu_baseline): 16.8 M cell-updates, about 15 core-seconds")
+    ap.add_argument("--ref-groups", type=int, default=2048, help="groups per step of the --impl reference arm")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-multistep", action="store_true")
