@@ -148,7 +148,7 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-multistep", action="store_true")
-    ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused", "fused_scalar", "fused_pair"],
+    ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused", "fused_scalar", "fused_duo"],
                     help="kernel path forced through gamer_hydro_set_path (default: the library's choice)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -175,7 +175,7 @@ def main():
     G = groups.shape[0]
     cells = G * N ** 3
     gh.gamer_hydro_alloc(G, N, GHOST, 4, local_rank)
-    gh.gamer_hydro_set_path({"auto": 0, "generic": 1, "fused": 2, "fused_scalar": 3, "fused_pair": 4}[args.path])
+    gh.gamer_hydro_set_path({"auto": 0, "generic": 1, "fused": 2, "fused_scalar": 3, "fused_duo": 4}[args.path])
     h_in = torch.from_numpy(groups)
     d_in = h_in.to(dev)
     d_out = torch.empty((G, 5, N, N, N), dtype=torch.float32, device=dev)

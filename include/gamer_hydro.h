@@ -46,16 +46,17 @@ enum {
 enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1 };
 
 /* kernel selection for gamer_hydro_set_path: AUTO picks FUSED when N == 16, else GENERIC. FUSED is the
- * performance path (fp32: one cell per thread, the two lanes of every packed f32x2 instruction carry two
- * directions of the cell; fp64: one cell per thread, scalar). FUSED_SCALAR forces the scalar fused kernel in
- * fp32 as well and FUSED_PAIR the two-cells-per-thread packed kernel: two more, structurally different,
- * implementations of the same step (tests, comparisons). */
+ * performance path (fp32: one column per thread, the two lanes of every packed f32x2 instruction carry two
+ * consecutive z planes; fp64: one cell per thread, scalar). FUSED_SCALAR forces the scalar fused kernel in
+ * fp32 as well and FUSED_DUO the one-cell-per-thread kernel whose packed lanes carry two directions (the
+ * kernel the fused-halo step of gamer_hydro_step_grid is built on): structurally different implementations
+ * of the same step (tests, comparisons). */
 enum {
   GAMER_HYDRO_PATH_AUTO = 0,
   GAMER_HYDRO_PATH_GENERIC = 1,
   GAMER_HYDRO_PATH_FUSED = 2,
   GAMER_HYDRO_PATH_FUSED_SCALAR = 3,
-  GAMER_HYDRO_PATH_FUSED_PAIR = 4
+  GAMER_HYDRO_PATH_FUSED_DUO = 4
 };
 
 /* One-time, idempotent, process-global set-up for `device`: checks the compute capability, raises the

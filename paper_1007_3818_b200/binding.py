@@ -15,7 +15,7 @@ _LIB_PATH = os.path.join(_HERE, "libgamer_hydro.so")
 _lib = None
 
 MINMOD, VANLEER = 0, 1
-PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_PAIR = 0, 1, 2, 3, 4
+PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_DUO = 0, 1, 2, 3, 4
 
 EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",

@@ -13,8 +13,9 @@
 #include "../../include/gamer_hydro.h"
 #include "hydro_fused.cuh"
 #include "hydro_generic.cuh"
-#include "hydro_pair.cuh"
+#include "hydro_f2.cuh"
 #include "hydro_duo.cuh"
+#include "hydro_zpair.cuh"
 #include "hydro_aux.cuh"
 
 namespace {
@@ -88,8 +89,8 @@ int init_locked(int device) {
   if ((rc = set_fused_attr<float, 1, true>())) return rc;
   if ((rc = set_fused_attr<double, 0, false>())) return rc;
   if ((rc = set_fused_attr<double, 1, false>())) return rc;
-  CK(cudaFuncSetAttribute(gh::pair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
-  CK(cudaFuncSetAttribute(gh::pair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::PairSmem::total));
+  CK(cudaFuncSetAttribute(gh::zpair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::ZSmem::total));
+  CK(cudaFuncSetAttribute(gh::zpair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::ZSmem::total));
   CK(cudaFuncSetAttribute(gh::duo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_halo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
@@ -156,14 +157,15 @@ bool fused_supported(int N, int ghost) {
   return N == gh::FN && ((S * (int)sizeof(R)) % 16 == 0) && (((ghost - 2) * (int)sizeof(R)) % 16 == 0);
 }
 
-// rank-5 tensor map (x, y, z, var, group) over U_in; box = one z plane of all five variables (20 x 20 x 1 x 5 x 1)
+// rank-5 tensor map (x, y, z, var, group) over U_in; box = box_z consecutive z planes of all five variables
+// (20 x 20 x box_z x 5 x 1); planes outside the array are zero-filled
 template <class R>
-int encode_plane_map(const R* U_in, int n_groups, int N, int ghost, CUtensorMap& map) {
+int encode_plane_map(const R* U_in, int n_groups, int N, int ghost, CUtensorMap& map, int box_z = 1) {
   const int S = N + 2 * ghost;
   const cuuint64_t dims[5] = {(cuuint64_t)S, (cuuint64_t)S, (cuuint64_t)S, 5, (cuuint64_t)n_groups};
   const cuuint64_t strides[4] = {(cuuint64_t)S * sizeof(R), (cuuint64_t)S * S * sizeof(R),
                                  (cuuint64_t)S * S * S * sizeof(R), (cuuint64_t)5 * S * S * S * sizeof(R)};
-  const cuuint32_t box[5] = {(cuuint32_t)gh::FS, (cuuint32_t)gh::FS, 1, 5, 1};
+  const cuuint32_t box[5] = {(cuuint32_t)gh::FS, (cuuint32_t)gh::FS, (cuuint32_t)box_z, 5, 1};
   const cuuint32_t estr[5] = {1, 1, 1, 1, 1};
   const CUtensorMapDataType dt_ = sizeof(R) == 4 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT32 : CU_TENSOR_MAP_DATA_TYPE_FLOAT64;
   CUresult r = g_state.encode(&map, dt_, 5, const_cast<R*>(U_in), dims, strides, box, estr,
@@ -226,21 +228,18 @@ int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int 
   return 0;
 }
 
-// fp32, two cells per thread with packed f32x2 arithmetic (hydro_pair.cuh); selectable, not the default
-int launch_pair(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
-                float gamma, int limiter, cudaStream_t stream) {
+// fp32 default: one column per thread, the f32x2 lanes carry two consecutive z planes (hydro_zpair.cuh)
+int launch_zpair(const float* U_in, float* U_out, float* bflux, int n_groups, int N, int ghost, float dt, float dx,
+                 float gamma, int limiter, cudaStream_t stream) {
   CUtensorMap map;
-  int rc = encode_plane_map<float>(U_in, n_groups, N, ghost, map);
+  int rc = encode_plane_map<float>(U_in, n_groups, N, ghost, map, 2);
   if (rc) return rc;
   const gh::PairConst c = gh::make_pair_consts(dt, dx, gamma);
-  const int smem = gh::PairSmem::total;
-  const int per_sm = (2 * (smem + 1024) <= g_state.smem_per_sm) ? 2 : 1;
-  const int resident = g_state.sm_count * per_sm;
-  const int grid = n_groups < resident ? n_groups : resident;
+  const int grid = n_groups < g_state.sm_count ? n_groups : g_state.sm_count;   // persistent: one CTA per SM
   if (limiter == 0)
-    gh::pair_kernel<0><<<grid, gh::PNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+    gh::zpair_kernel<0><<<grid, gh::ZNT, gh::ZSmem::total, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
   else
-    gh::pair_kernel<1><<<grid, gh::PNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+    gh::zpair_kernel<1><<<grid, gh::ZNT, gh::ZSmem::total, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   return 0;
@@ -284,12 +283,12 @@ int step_impl(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost,
   int path = g_state.path;
   if (path == GAMER_HYDRO_PATH_AUTO)
     path = fused_supported<R>(N, ghost) ? GAMER_HYDRO_PATH_FUSED : GAMER_HYDRO_PATH_GENERIC;
-  if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR || path == GAMER_HYDRO_PATH_FUSED_PAIR) {
+  if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR || path == GAMER_HYDRO_PATH_FUSED_DUO) {
     if (!fused_supported<R>(N, ghost)) return GAMER_HYDRO_UNSUPPORTED;
     if constexpr (sizeof(R) == 4) {
-      if (path == GAMER_HYDRO_PATH_FUSED_PAIR)
-        return launch_pair(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
       if (path == GAMER_HYDRO_PATH_FUSED)
+        return launch_zpair(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+      if (path == GAMER_HYDRO_PATH_FUSED_DUO)
         return launch_duo(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
     }
     return launch_fused<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
@@ -569,7 +568,7 @@ int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonp
 }
 
 int gamer_hydro_set_path(int path) {
-  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_PAIR) return GAMER_HYDRO_INVALID_ARG;
+  if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_DUO) return GAMER_HYDRO_INVALID_ARG;
   g_state.path = path;
   return 0;
 }
@@ -586,12 +585,5 @@ const char* gamer_hydro_strerror(int code) {
     default: return "unknown error code";
   }
 }
-
-#ifdef GH_PROBE
-int gamer_hydro_probe(unsigned long long* out) {
-  cudaDeviceSynchronize();
-  return (int)cudaMemcpyFromSymbol(out, gh::gh_probe, sizeof(unsigned long long) * 80);
-}
-#endif
 
 }  // extern "C"

@@ -15,7 +15,7 @@
 #include <cuda.h>
 #include <stdint.h>
 
-#include "hydro_pair.cuh"  // f2 helpers, PairConst, St2, roe2, limiters, mbarrier / TMA helpers
+#include "hydro_f2.cuh"  // f2 helpers, PairConst, St2, roe2, limiters, mbarrier / TMA helpers
 
 namespace gh {
 
@@ -127,13 +127,6 @@ __device__ __forceinline__ void roe1_z(const St1& L, const St1& R, float g1, flo
   F[1] = fmaf(0.5f, fmaf(mL, L.u, mR * R.u), Dt1);
   F[2] = fmaf(0.5f, fmaf(mL, L.v, mR * R.v), Dt2);
   F[4] = fmaf(0.5f, fmaf(mL, L.h, mR * R.h), D4);
-}
-
-template <int LIM>
-__device__ __forceinline__ float limited_slope1(float a, float b) {
-  if (LIM == 0) return minmod1(a, b);
-  const float p = a * b, s = a + b;
-  return vanleer1(a, b, p, s);
 }
 
 // One half-CTA (320 threads). HALF is a template parameter so that every shared-memory address and the named

@@ -14,7 +14,7 @@ from paper_1007_3818_b200 import workloads as wl
 pytestmark = pytest.mark.gpu
 G = wl.GAMMA
 TOL32_1, TOL32_10, TOL64 = 1e-4, 1e-3, 1e-11
-PATHS = [gh.PATH_FUSED, gh.PATH_GENERIC, gh.PATH_FUSED_PAIR, gh.PATH_FUSED_SCALAR]
+PATHS = [gh.PATH_FUSED, gh.PATH_GENERIC, gh.PATH_FUSED_DUO, gh.PATH_FUSED_SCALAR]
 
 
 def check(groups, dt, dx, limiter, path, tol, gamma=G, max_excl=pu.MAX_EXCLUDED_FRACTION, ghost=2):
@@ -299,7 +299,7 @@ def test_headline_full_size_in_the_bench_launch_configuration():
     assert guard_gpu > 0
 
 
-@pytest.mark.parametrize("path", [gh.PATH_FUSED, gh.PATH_FUSED_PAIR, gh.PATH_FUSED_SCALAR])
+@pytest.mark.parametrize("path", [gh.PATH_FUSED, gh.PATH_FUSED_DUO, gh.PATH_FUSED_SCALAR])
 def test_repeated_launches_are_bit_identical(path):
     """Race stress for the split-barrier / double-buffer protocols of the fused kernels: 4096 groups (14 per
     persistent CTA, so every buffer is recycled hundreds of times) launched 25 times must give the same bits every
