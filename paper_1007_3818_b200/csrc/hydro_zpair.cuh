@@ -16,8 +16,8 @@
 //   warps 0..7  interior cells, j = t / 16, i = t % 16 (a half-warp = one row: 64-bit accesses are conflict-free)
 //   warp  8     "upper" ghosts: column i = 16 (lanes 0..15) and row j = 16 (lanes 16..31): own '-' state along the
 //               normal + the Roe solve of the face they own
-//   warp  9     "lower" ghosts: column i = -1 and row j = -1: own '+' state along the normal; also the TMA producer,
-//               the 68 neighbour-only cells of the conversion and the x / y boundary-flux stores
+//   warp  9     "lower" ghosts: column i = -1 and row j = -1: own '+' state along the normal; also the TMA producer
+//               and the x / y boundary-flux stores (the 68 neighbour-only cells of the conversion go to warps 2, 3, 6, 7)
 // Ghost lanes work in a ROTATED frame (normal, tangential, z): only shared-memory offsets differ between the lanes.
 // Per slot s (plane pair s of the flat sequence; everything a neighbour publishes is double-buffered):
 //   C  cons -> prim of pair s+1 (raw pairs arrive by TMA: box 20 x 20 x 2 x 5, ring of ZNS stages) -> W[(s+1)&1]
@@ -41,7 +41,11 @@
 
 namespace gh {
 
-constexpr int ZNT = 320;            // threads per CTA
+#ifndef GH_ZNT
+#define GH_ZNT 320
+#endif
+constexpr int ZNT = GH_ZNT;         // threads per CTA: 8 interior warps + 2 ghost warps (320), or + 2 x 2 ghost warps that alternate slots (384)
+constexpr bool ZROT = ZNT == 384;
 constexpr int ZNW = ZNT / 32;       // warps (arrival count of the split barriers)
 #ifndef GH_ZNS
 #define GH_ZNS 5
@@ -67,6 +71,21 @@ struct ZSmem {
   static constexpr int total = off_bar + (ZNS + 2) * 8;
 };
 static_assert(ZSmem::total <= 232448, "z-pair kernel: shared memory over the 227 KB limit");
+
+// wait with a suspend-time hint: the warp sleeps in hardware until the phase completes (or the hint expires) instead
+// of polling — the polls of waiting warps take issue slots from the working warps of the same scheduler
+__device__ __forceinline__ void mbar_wait_sleep(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1, %2;\n"
+      "@p bra DONE_%=;\n"
+      "bra WAIT_%=;\n"
+      "DONE_%=:\n"
+      "}\n" ::"r"(bar), "r"(parity), "r"(20000u)
+      : "memory");
+}
 
 __device__ __forceinline__ void tma_load_pair(uint32_t dst, const CUtensorMap* map, int x, int y, int z, int g, uint32_t bar) {
   asm volatile(
@@ -157,8 +176,9 @@ __device__ __forceinline__ St2 zp_state(const f2 Uf[5], const f2 dU[5], const Pa
   return o;
 }
 
-// ROLE 0: interior warps; 1: upper ghosts (warp 8); 2: lower ghosts (warp 9)
-template <int LIM, int ROLE>
+// One instruction stream for all ten warps (the three roles differ in a few warp-uniform branches and in per-lane
+// shared-memory offsets only): role 0 = interior warps; 1 = upper ghosts (warp 8); 2 = lower ghosts (warp 9)
+template <int LIM>
 __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restrict__ U_out, float* __restrict__ bflux,
                                        int n_groups, int goff, const PairConst& c,
                                        unsigned long long* __restrict__ status, unsigned char* smem) {
@@ -172,25 +192,33 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
 
   // ---- thread -> column (i, j); ghost lanes: rot = the normal is y
   const int t = (int)threadIdx.x, lane = t & 31;
+  const int role = t < 256 ? 0 : 1 + ((t >> 5) & 1);       // warp-uniform: warps 8, 10 upper ghosts, 9, 11 lower ghosts
+  const int duty_par = t >= 320 ? 1 : 0;                   // ghost warps 8, 9 work in the even slots, 10, 11 in the odd ones
   int i, j;
   bool rot = false;
-  if (ROLE == 0) { j = t >> 4; i = t & 15; }
+  if (role == 0) { j = t >> 4; i = t & 15; }
   else {
     const int l = lane & 15;
     rot = lane >= 16;
-    if (ROLE == 1) { i = rot ? l : FN; j = rot ? FN : l; }
+    if (role == 1) { i = rot ? l : FN; j = rot ? FN : l; }
     else { i = rot ? l : -1; j = rot ? -1 : l; }
   }
   const int w_own = 2 * ((j + 2) * ZWP + (i + 2));          // float offsets (8-byte elements)
   const int raw_own = (j + 2) * FS + (i + 2);
   // neighbour strides and the component planes holding the normal / tangential velocity (float offsets)
-  const int offn = (ROLE == 0) ? 2 : (rot ? 2 * ZWP : 2);
-  const int offt = (ROLE == 0) ? 2 * ZWP : (rot ? 2 : 2 * ZWP);
-  const int cq1 = (ROLE == 0) ? 2 * ZWQ : (rot ? 4 * ZWQ : 2 * ZWQ);
-  const int cq2 = (ROLE == 0) ? 4 * ZWQ : (rot ? 2 * ZWQ : 4 * ZWQ);
+  const int offn = rot ? 2 * ZWP : 2;
+  const int offt = rot ? 2 : 2 * ZWP;
+  const int cq1 = rot ? 4 * ZWQ : 2 * ZWQ;
+  const int cq2 = rot ? 2 * ZWQ : 4 * ZWQ;
   auto wq = [&](int q) { return q == 1 ? cq1 : (q == 2 ? cq2 : 2 * q * ZWQ); };
   // exchange arrays of one pair: [SX: 6 x ZNX][SY: 6 x ZNY] and [FX: 5 x ZNX][FY: 5 x ZNY], 8-byte elements
   const int ix = 2 * (i + 17 * j), iy = 2 * (i + 16 * j);   // own lower x / y face (float offsets)
+  // where the '+' state along the first direction is published: x+ of cell (i, j) -> SX[(i+1) + 17 j]; a rotated
+  // ghost lane's y+ -> SY[i + 16 (j+1)] with the slots of u and v exchanged
+  const bool p1y = rot;
+  const int p1o = rot ? iy + 2 * FN : ix + 2;
+  const int p1s = rot ? 2 * ZNY : 2 * ZNX;
+  const int p1u = rot ? 2 * p1s : p1s, p1v = rot ? p1s : 2 * p1s;
 
   const int n_local = (n_groups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int n_slots = n_local * ZSLOTS;
@@ -210,7 +238,7 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
       if (++iss_stage == ZNS) iss_stage = 0;
     }
   };
-  const bool producer = (ROLE == 2) && lane == 0;
+  const bool producer = t == 288;
   if (producer) issue_upto(ZNS);
 
   uint32_t s_phase = 0, f_phase = 1;   // the first wait(F) passes on the fresh barrier
@@ -226,6 +254,7 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
     if (++c_stage == ZNS) { c_stage = 0; c_par ^= 1u; }
     return p;
   };
+  auto skip_raw = [&]() { if (++c_stage == ZNS) { c_stage = 0; c_par ^= 1u; } };
   auto convert = [&](const float* raw, int off, f2 W[5]) {
     f2 U[5];
 #pragma unroll
@@ -244,8 +273,8 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
     f2 W[5];
     convert(next_raw(), raw_own, W);
     Wc[0] = W[0]; Wc[3] = W[3]; Wc[4] = W[4];
-    Wc[1] = (ROLE != 0 && rot) ? W[2] : W[1];
-    Wc[2] = (ROLE != 0 && rot) ? W[1] : W[2];
+    Wc[1] = rot ? W[2] : W[1];
+    Wc[2] = rot ? W[1] : W[2];
 #pragma unroll
     for (int q = 0; q < 5; ++q) az[q] = 0.0f;
   }
@@ -256,51 +285,47 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   float dzlo[5], Fzh[5];
 #pragma unroll
   for (int q = 0; q < 5; ++q) { accxy[q] = c.one; dzlo[q] = 0.0f; Fzh[q] = 0.0f; }
-  f2 dzz[5];                                         // (Fz_up - Fz_lo) of the pair awaiting its update
-#pragma unroll
-  for (int q = 0; q < 5; ++q) dzz[q] = c.one;
 
   // The slot body is written as straight-line PHASES (lambdas, inlined) so that each region between two barrier
   // operations is one basic block the scheduler can interleave: {C, P}, {Z, U}, {R, reload}. Slot-dependent special
   // cases (the two light slots of a group, the first / last update, boundary-flux stores) live in warp-uniform side
   // branches.
   int gs = 0, g = (int)blockIdx.x;
-  float cz[5];                                       // W(lower plane of pair s+1) - W(upper plane of pair s)
-  St2 Sm1, Sm2;                                      // interior: x- and y- states; upper ghosts: Sm1 = the normal '-' state
-  St2 Szm, Szp;                                      // interior: z- and z+ states
 
   // ---- C: primitives of pair s+1 -> W[(s+1)&1]
-  auto phaseC = [&](float* w_nxt) {
+  // cz: W(lower plane of pair s+1) - W(upper plane of pair s)
+  auto phaseC = [&](float* w_nxt, float cz[5]) {
     const float* raw = next_raw();
     f2 Wn[5];
     convert(raw, raw_own, Wn);
 #pragma unroll
     for (int q = 0; q < 5; ++q) sts2(w_nxt + w_own + 2 * q * ZWQ, Wn[q]);
-    if (ROLE == 2) {  // the 68 cells of a plane that are only ever neighbours: rows -2 / 17, columns -2 / 17, inner corners
+    if (role == 0 && (t & 64)) {
+      // the 68 cells of a plane that are only ever neighbours (rows -2 / 17, columns -2 / 17, inner corners): 17 each for
+      // the interior warps 2, 3, 6, 7 — the warps on the two schedulers that carry no ghost warp
+      const int e = 17 * (((t >> 7) << 1) | ((t >> 5) & 1)) + lane;
+      if (lane < 17) {
+        int ei, ej;
+        if (e < 32) { ei = e & 15; ej = (e < 16) ? -2 : FN + 1; }
+        else if (e < 64) { ej = e & 15; ei = (e < 48) ? -2 : FN + 1; }
+        else { ei = (e & 1) ? FN : -1; ej = (e & 2) ? FN : -1; }
+        f2 We[5];
+        convert(raw, (ej + 2) * FS + (ei + 2), We);
+        float* we = w_nxt + 2 * ((ej + 2) * ZWP + (ei + 2));
 #pragma unroll
-      for (int r = 0; r < 3; ++r) {
-        const int e = lane + 32 * r;
-        if (e < 68) {
-          int ei, ej;
-          if (e < 32) { ei = e & 15; ej = (e < 16) ? -2 : FN + 1; }
-          else if (e < 64) { ej = e & 15; ei = (e < 48) ? -2 : FN + 1; }
-          else { ei = (e & 1) ? FN : -1; ej = (e & 2) ? FN : -1; }
-          f2 We[5];
-          convert(raw, (ej + 2) * FS + (ei + 2), We);
-          float* we = w_nxt + 2 * ((ej + 2) * ZWP + (ei + 2));
-#pragma unroll
-          for (int q = 0; q < 5; ++q) sts2(we + 2 * q * ZWQ, We[q]);
-        }
+        for (int q = 0; q < 5; ++q) sts2(we + 2 * q * ZWQ, We[q]);
       }
     }
-    const float n1 = (ROLE != 0 && rot) ? lo(Wn[2]) : lo(Wn[1]);
-    const float n2 = (ROLE != 0 && rot) ? lo(Wn[1]) : lo(Wn[2]);
+    const float n1 = rot ? lo(Wn[2]) : lo(Wn[1]);
+    const float n2 = rot ? lo(Wn[1]) : lo(Wn[2]);
     cz[0] = lo(Wn[0]) - hi(Wc[0]); cz[1] = n1 - hi(Wc[1]); cz[2] = n2 - hi(Wc[2]);
     cz[3] = lo(Wn[3]) - hi(Wc[3]); cz[4] = lo(Wn[4]) - hi(Wc[4]);
   };
 
   // ---- P: reconstruction + half-step prediction of the pair; publishes the x+ / y+ states into S[buf]
-  auto phaseP = [&](const float* w_cur, float* sx, float* sy) {
+  // Sm1, Sm2: the '-' states along the two in-plane directions (interior: x-, y-; upper ghosts use Sm1); Szm, Szp: z-, z+
+  auto phaseP = [&](const float* w_cur, float* sx, float* sy, const float cz[5], St2& Sm1, St2& Sm2, St2& Szm, St2& Szp) {
+    float* const p1 = (p1y ? sy : sx) + p1o;
     f2 s1[5], s2[5], s3[5];
     {
       const float* wp = w_cur + w_own;
@@ -325,85 +350,64 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
       for (int q = 0; q < 5; ++q) dU[q] = c.hlamn * acc[q];
     }
     f2 gmin = c.one;
-    if (ROLE == 0) {
-      {
-        const St2 S = zp_state<+1>(U1p, dU, c, gmin);   // x+ : left state of the face i + 1/2
-        float* o = sx + ix + 2;
-        sts2(o, S.r); sts2(o + 2 * ZNX, S.u); sts2(o + 4 * ZNX, S.v); sts2(o + 6 * ZNX, S.w);
-        sts2(o + 8 * ZNX, S.p); sts2(o + 10 * ZNX, S.h);
+    // '+' states along the first / second in-plane direction: published where a neighbour needs them — interior: x+ ->
+    // SX[(i+1) + 17 j], y+ -> SY[i + 16 (j+1)]; lower ghosts: the normal one -> SX[17 j] / SY[i], rotated slots
+    {
+      const St2 S = zp_state<+1>(U1p, dU, c, gmin);
+      if (role != 1) {
+        float* o = p1;
+        sts2(o, S.r); sts2(o + p1u, S.u); sts2(o + p1v, S.v); sts2(o + 3 * p1s, S.w);
+        sts2(o + 4 * p1s, S.p); sts2(o + 5 * p1s, S.h);
       }
-      {
-        const St2 S = zp_state<+1>(U2p, dU, c, gmin);   // y+
+    }
+    {
+      const St2 S = zp_state<+1>(U2p, dU, c, gmin);
+      if (role == 0) {
         float* o = sy + iy + 2 * FN;
         sts2(o, S.r); sts2(o + 2 * ZNY, S.u); sts2(o + 4 * ZNY, S.v); sts2(o + 6 * ZNY, S.w);
         sts2(o + 8 * ZNY, S.p); sts2(o + 10 * ZNY, S.h);
       }
-      Sm1 = zp_state<-1>(U1m, dU, c, gmin);
-      Sm2 = zp_state<-1>(U2m, dU, c, gmin);
-      Szm = zp_state<-1>(U3m, dU, c, gmin);
-      Szp = zp_state<+1>(U3p, dU, c, gmin);
-      const bool ok_lo = lo(gmin) > 0.0f, ok_hi = hi(gmin) > 0.0f;
-      if (__builtin_expect(!(ok_lo && ok_hi), 0)) {
-        // rare: first-order fallback (reading R7) — all six states of the failing cell become its own input state
-        f2 W0[5];
-        load_own(w_cur, W0);
-        St2 fb;
-        fb.r = W0[0]; fb.u = W0[1]; fb.v = W0[2]; fb.w = W0[3]; fb.p = W0[4];
-        const f2 q = fma2(W0[3], W0[3], fma2(W0[2], W0[2], W0[1] * W0[1]));
-        fb.h = fma2(c.half, q, (c.gg1 * W0[4]) * rcp2(W0[0]));
-        fix_state(Sm1, ok_lo, ok_hi, fb); fix_state(Sm2, ok_lo, ok_hi, fb);
-        fix_state(Szm, ok_lo, ok_hi, fb); fix_state(Szp, ok_lo, ok_hi, fb);
-        const float fl[6] = {lo(fb.r), lo(fb.u), lo(fb.v), lo(fb.w), lo(fb.p), lo(fb.h)};
-        const float fh[6] = {hi(fb.r), hi(fb.u), hi(fb.v), hi(fb.w), hi(fb.p), hi(fb.h)};
-        float* ox = sx + ix + 2;
-        float* oy = sy + iy + 2 * FN;
+    }
+    Sm1 = zp_state<-1>(U1m, dU, c, gmin);
+    Sm2 = zp_state<-1>(U2m, dU, c, gmin);
+    Szm = zp_state<-1>(U3m, dU, c, gmin);
+    Szp = zp_state<+1>(U3p, dU, c, gmin);
+    // all six states enter the guard (as in the oracle), also in the ghost columns that use one of them; the ghost
+    // columns of the two ghost planes (-1: lower lane of the first pair, 16: upper lane of the last) are never used
+    const bool ok_lo = lo(gmin) > 0.0f || (role != 0 && gs == 1), ok_hi = hi(gmin) > 0.0f || (role != 0 && gs == 9);
+    if (__builtin_expect(!(ok_lo && ok_hi), 0)) {
+      // rare: first-order fallback (reading R7) — all six states of the failing cell become its own input state
+      f2 W0[5];
+      load_own(w_cur, W0);
+      St2 fb;
+      fb.r = W0[0]; fb.u = W0[1]; fb.v = W0[2]; fb.w = W0[3]; fb.p = W0[4];
+      const f2 q = fma2(W0[3], W0[3], fma2(W0[2], W0[2], W0[1] * W0[1]));
+      fb.h = fma2(c.half, q, (c.gg1 * W0[4]) * rcp2(W0[0]));
+      fix_state(Sm1, ok_lo, ok_hi, fb); fix_state(Sm2, ok_lo, ok_hi, fb);
+      fix_state(Szm, ok_lo, ok_hi, fb); fix_state(Szp, ok_lo, ok_hi, fb);
+      const float fl[6] = {lo(fb.r), lo(fb.u), lo(fb.v), lo(fb.w), lo(fb.p), lo(fb.h)};
+      const float fh[6] = {hi(fb.r), hi(fb.u), hi(fb.v), hi(fb.w), hi(fb.p), hi(fb.h)};
+      const int so[6] = {0, p1u, p1v, 3 * p1s, 4 * p1s, 5 * p1s};
+      float* oy = sy + iy + 2 * FN;
 #pragma unroll
-        for (int m = 0; m < 6; ++m) {
-          if (!ok_lo) { ox[2 * m * ZNX] = fl[m]; oy[2 * m * ZNY] = fl[m]; }
-          if (!ok_hi) { ox[2 * m * ZNX + 1] = fh[m]; oy[2 * m * ZNY + 1] = fh[m]; }
+      for (int m = 0; m < 6; ++m) {
+        if (role != 1) {
+          if (!ok_lo) p1[so[m]] = fl[m];
+          if (!ok_hi) p1[so[m] + 1] = fh[m];
         }
-        n_guard += (ok_lo ? 0u : 1u) + (ok_hi ? 0u : 1u);   // both planes of an interior column are cells whose states are used
+        if (role == 0) {
+          if (!ok_lo) oy[2 * m * ZNY] = fl[m];
+          if (!ok_hi) oy[2 * m * ZNY + 1] = fh[m];
+        }
       }
-    } else {
-      // ghost lanes: all six states enter the guard (as in the oracle), one of them is used
-      St2 Su;
-      if (ROLE == 1) {
-        (void)zp_state<+1>(U1p, dU, c, gmin);
-        Su = zp_state<-1>(U1m, dU, c, gmin);
-      } else {
-        Su = zp_state<+1>(U1p, dU, c, gmin);
-        (void)zp_state<-1>(U1m, dU, c, gmin);
-      }
-      (void)zp_state<+1>(U2p, dU, c, gmin); (void)zp_state<-1>(U2m, dU, c, gmin);
-      (void)zp_state<+1>(U3p, dU, c, gmin); (void)zp_state<-1>(U3m, dU, c, gmin);
-      // the ghost cells of the two ghost planes (-1: lower lane of the first pair, 16: upper lane of the last) are never used
-      const bool ok_lo = lo(gmin) > 0.0f || gs == 1, ok_hi = hi(gmin) > 0.0f || gs == 9;
-      if (__builtin_expect(!(ok_lo && ok_hi), 0)) {
-        f2 W0[5];
-        load_own(w_cur, W0);
-        St2 fb;
-        fb.r = W0[0]; fb.u = W0[1]; fb.v = W0[2]; fb.w = W0[3]; fb.p = W0[4];
-        const f2 q = fma2(W0[3], W0[3], fma2(W0[2], W0[2], W0[1] * W0[1]));
-        fb.h = fma2(c.half, q, (c.gg1 * W0[4]) * rcp2(W0[0]));
-        fix_state(Su, ok_lo, ok_hi, fb);
-        n_guard += (ok_lo ? 0u : 1u) + (ok_hi ? 0u : 1u);
-      }
-      if (ROLE == 2) {
-        // publish the '+' state along the normal: x+ of cell (-1, j) -> SX[0 + 17 j]; y+ of cell (i, -1) -> SY[i]
-        float* o = rot ? (sy + 2 * i) : (sx + 2 * 17 * j);
-        const int st = rot ? 2 * ZNY : 2 * ZNX;
-        const int s1o = rot ? 2 * st : st, s2o = rot ? st : 2 * st;   // slots of the normal / tangential velocity
-        sts2(o, Su.r); sts2(o + s1o, Su.u); sts2(o + s2o, Su.v); sts2(o + 3 * st, Su.w);
-        sts2(o + 4 * st, Su.p); sts2(o + 5 * st, Su.h);
-      } else {
-        Sm1 = Su;
-      }
+      n_guard += (ok_lo ? 0u : 1u) + (ok_hi ? 0u : 1u);   // every cell that gets here is one whose states are used
     }
   };
 
   // ---- Z (interior): the two lower z faces of the pair; left states (z+ of the plane below, z+ of the pair's lower
   // plane). The pair awaiting its update (slot s-1) gets its last z difference; this pair starts its own.
-  auto phaseZ = [&]() {
+  // dzz: (Fz_up - Fz_lo) of the pair awaiting its update
+  auto phaseZ = [&](const St2& Szm, const St2& Szp, f2 dzz[5]) {
     St2 Lq;
     Lq.r = mk2(Lz[0], lo(Szp.r)); Lq.u = mk2(Lz[1], lo(Szp.u)); Lq.v = mk2(Lz[2], lo(Szp.v));
     Lq.w = mk2(Lz[3], lo(Szp.w)); Lq.p = mk2(Lz[4], lo(Szp.p)); Lq.h = mk2(Lz[5], lo(Szp.h));
@@ -420,10 +424,10 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
 
   // ---- U: conservative update of pair s-1 (planes k_lo = 2 gs - 5, k_hi = 2 gs - 4) from F[buf ^ 1]; VLO / VHI: which
   // of the two planes is an interior one (both, except in the first and the last update of a group)
-  auto phaseU = [&](auto vlo_c, auto vhi_c, const float* fx, const float* fy, float* outg, float* bfg) {
+  auto phaseU = [&](auto vlo_c, auto vhi_c, const float* fx, const float* fy, float* outg, float* bfg, const f2 dzz[5]) {
     constexpr bool VLO = decltype(vlo_c)::value, VHI = decltype(vhi_c)::value;
     const int k_lo = 2 * gs - 5;
-    if (ROLE == 0) {
+    if (role == 0) {
       const float* rawp = reinterpret_cast<const float*>(smem + SM::off_raw + u_stage * SM::raw_stage_bytes) + raw_own;
       float* op = outg + k_lo * (FN * FN) + j * FN + i;
       f2 out[5];
@@ -443,7 +447,7 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
       if (VLO) n_nonpos += ((lo(out[0]) > 0.0f) & (lo(tre) > lo(m2))) ? 0u : 1u;
       if (VHI) n_nonpos += ((hi(out[0]) > 0.0f) & (hi(tre) > hi(m2))) ? 0u : 1u;
     }
-    if (ROLE == 2 && bfg) {
+    if (role == 2 && bfg) {
       // a5: the x / y boundary fluxes of pair s-1, from the flux arrays: lanes 0..15 the lower face, 16..31 the upper
       const int l = lane & 15, side = lane >> 4;
       const float* px = fx + 2 * (side * FN + 17 * l);
@@ -462,8 +466,8 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   using F_ = std::false_type;
 
   // ---- R: Roe fluxes at the lower x and the lower y face of the pair -> F[buf]
-  auto phaseR = [&](const float* sx, const float* sy, float* fx, float* fy) {
-    if (ROLE == 0) {
+  auto phaseR = [&](const float* sx, const float* sy, float* fx, float* fy, const St2& Sm1, const St2& Sm2) {
+    if (role == 0) {
       f2 Fx[5], Fy[5];
       St2 Lx, Ly;
       {
@@ -482,7 +486,7 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
         sts2(fy + 2 * q * ZNY + iy, Fy[q]);
         accxy[q] = Fx[q] + Fy[q];
       }
-    } else if (ROLE == 1) {
+    } else if (role == 1) {
       // the face this ghost owns: x = 15.5 (column i = 16) or y = 15.5 (row j = 16), solved in the rotated frame
       const float* p = rot ? (sy + iy) : (sx + ix);
       const int st = rot ? 2 * ZNY : 2 * ZNX;
@@ -511,48 +515,72 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
     const float* const fxp = fbase + (buf ^ 1) * (SM::f_bytes / 4);   // fluxes of slot s-1
     const float* const fyp = fxp + 10 * ZNX;
 
-    if (gs >= 1 && gs <= 9) {
-      // ================= a full slot: the pair (2 gs - 3, 2 gs - 2) =================
-      phaseC(w_nxt);
-      phaseP(w_cur, sx, sy);
-      warp_arrive(s_bar);                    // everything the neighbours need from this warp is published
-      mbar_wait(f_bar, f_phase);             // every warp has finished slot s-1 (arrived at its end: long since)
+    // the ghost columns are served by two pairs of warps in alternate slots (the four schedulers then carry the same
+    // load); a ghost warp keeps no state between its slots: it re-reads its column from the primitive pair-planes
+    const bool duty = !ZROT || role == 0 || ((s & 1) == duty_par);
+    auto wait_f = [&]() {
+      mbar_wait_sleep(f_bar, f_phase);       // every warp has finished slot s-1 (arrived at its end: long since)
       f_phase ^= 1u;
       if (producer) issue_upto(s - 1 + ZNS); // pairs <= s-2 are retired (their last reader is the update in slot s-1)
-      if (ROLE == 0) phaseZ();
-      if (gs >= 3) phaseU(T_{}, T_{}, fxp, fyp, outg, bfg);
-      else if (gs == 2) phaseU(F_{}, T_{}, fxp, fyp, outg, bfg);
-      if (ROLE == 0 && bfg && (gs == 1 || gs == 9)) {   // a5: faces -z (the upper face of plane -1) and +z (of plane 15)
-        float* p = bfg + (4 + (gs == 9)) * (5 * FN * FN) + j * FN + i;
-#pragma unroll
-        for (int q = 0; q < 5; ++q) p[q * (FN * FN)] = Fzh[q];
-      }
-      mbar_wait(s_bar, s_phase);             // x+ / y+ states of this pair and the primitives of pair s+1 are visible
+    };
+    auto wait_s = [&]() {
+      mbar_wait_sleep(s_bar, s_phase);       // x+ / y+ states of this pair and the primitives of pair s+1 are visible
       s_phase ^= 1u;
-      phaseR(sx, sy, fx, fy);
-    } else {
-      // ================= a light slot: gs = 0 (planes -3, -2) converts the first pair, gs = 10 finishes the last =====
-      phaseC(w_nxt);
-      warp_arrive(s_bar);
-      mbar_wait(f_bar, f_phase);
-      f_phase ^= 1u;
-      if (producer) issue_upto(s - 1 + ZNS);
-      if (gs == ZSLOTS - 1) {
-        if (ROLE == 0) {   // plane 16 gets no update; plane 15 needs the z difference it already has
+    };
+    if (duty) {
+      if (ZROT && role != 0) {
+        az[0] = w_nxt[w_own + 1];   // upper plane of pair s-1 (this warp's pair-plane of two slots ago, about to be overwritten)
+        az[1] = w_nxt[w_own + cq1 + 1]; az[2] = w_nxt[w_own + cq2 + 1];
+        az[3] = w_nxt[w_own + 6 * ZWQ + 1]; az[4] = w_nxt[w_own + 8 * ZWQ + 1];
+        load_own(w_cur, Wc);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) az[q] = lo(Wc[q]) - az[q];
+      }
+      float cz[5];
+      phaseC(w_nxt, cz);
+      if (gs >= 1 && gs <= 9) {
+        // ================= a full slot: the pair (2 gs - 3, 2 gs - 2) =================
+        St2 Sm1, Sm2, Szm, Szp;
+        phaseP(w_cur, sx, sy, cz, Sm1, Sm2, Szm, Szp);
+        warp_arrive(s_bar);                    // everything the neighbours need from this warp is published
+        wait_f();
+        f2 dzz[5];
+        if (role == 0) phaseZ(Szm, Szp, dzz);
+        if (gs >= 3) phaseU(T_{}, T_{}, fxp, fyp, outg, bfg, dzz);
+        else if (gs == 2) phaseU(F_{}, T_{}, fxp, fyp, outg, bfg, dzz);
+        if (role == 0 && bfg && (gs == 1 || gs == 9)) {   // a5: faces -z (the upper face of plane -1) and +z (of plane 15)
+          float* p = bfg + (4 + (gs == 9)) * (5 * FN * FN) + j * FN + i;
+#pragma unroll
+          for (int q = 0; q < 5; ++q) p[q * (FN * FN)] = Fzh[q];
+        }
+        wait_s();
+        phaseR(sx, sy, fx, fy, Sm1, Sm2);
+      } else {
+        // ================= a light slot: gs = 0 (planes -3, -2) converts the first pair, gs = 10 finishes the last =====
+        warp_arrive(s_bar);
+        wait_f();
+        if (gs == ZSLOTS - 1) {
+          f2 dzz[5];   // plane 16 gets no update; plane 15 needs the z difference it already has
 #pragma unroll
           for (int q = 0; q < 5; ++q) dzz[q] = mk2(dzlo[q], 0.0f);
+          phaseU(T_{}, F_{}, fxp, fyp, outg, bfg, dzz);
         }
-        phaseU(T_{}, F_{}, fxp, fyp, outg, bfg);
+        wait_s();
       }
-      mbar_wait(s_bar, s_phase);
-      s_phase ^= 1u;
+      // ---- next pair (interior): own column of W[(s+1)&1] (written by this thread in C), the z difference below it
+      if (!ZROT || role == 0) {
+        load_own(w_nxt, Wc);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) az[q] = cz[q];
+      }
+    } else {
+      skip_raw();
+      warp_arrive(s_bar);
+      wait_f();
+      wait_s();
     }
     warp_arrive(f_bar);
     if (++u_stage == ZNS) u_stage = 0;
-    // ---- next pair: own column of W[(s+1)&1] (written by this thread in C), the z difference below it
-    load_own(w_nxt, Wc);
-#pragma unroll
-    for (int q = 0; q < 5; ++q) az[q] = cz[q];
     if (++gs == ZSLOTS) { gs = 0; g += (int)gridDim.x; }
   }
 
@@ -580,10 +608,7 @@ __global__ void __launch_bounds__(ZNT, 1)
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   }
   __syncthreads();
-  const int warp = (int)threadIdx.x >> 5;
-  if (warp < 8) zp_run<LIM, 0>(in_map, U_out, bflux, n_groups, goff, c, status, zsmem);
-  else if (warp == 8) zp_run<LIM, 1>(in_map, U_out, bflux, n_groups, goff, c, status, zsmem);
-  else zp_run<LIM, 2>(in_map, U_out, bflux, n_groups, goff, c, status, zsmem);
+  zp_run<LIM>(in_map, U_out, bflux, n_groups, goff, c, status, zsmem);
 }
 
 }  // namespace gh
