@@ -462,10 +462,12 @@ int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, in
   double vmax = 0.0;
   int rc = gamer_hydro_max_speed(U, 4, (int)ng, N, ghost, (double)gamma, &vmax, stream);   // state on entry
   if (rc) return rc;
-  // Fully periodic grid of 16^3 groups on the default path: the step kernel itself writes the next step's ghosted
-  // array and signal-speed maximum (ping-pong between U and a library-owned second array). Otherwise: step + refill.
+  // Default: step + ghost refill (the refill pass also accumulates the next signal-speed maximum). With the DUO path
+  // selected, a fully periodic grid of 16^3 groups uses the fused-halo variant of that kernel instead: the step
+  // kernel itself writes the next step's ghosted array and signal-speed maximum (ping-pong between U and a
+  // library-owned second array).
   const bool fused_halo = bc_x == 0 && bc_y == 0 && bc_z == 0 && N == gh::FN && ghost == 2 &&
-                          (g_state.path == GAMER_HYDRO_PATH_AUTO || g_state.path == GAMER_HYDRO_PATH_FUSED);
+                          g_state.path == GAMER_HYDRO_PATH_FUSED_DUO;
   float* cur = U;
   float* nxt = nullptr;
   if (fused_halo) {

@@ -18,7 +18,9 @@
 //               normal + the Roe solve of the face they own
 //   warp  9     "lower" ghosts: column i = -1 and row j = -1: own '+' state along the normal; also the TMA producer
 //               and the x / y boundary-flux stores (the 68 neighbour-only cells of the conversion go to warps 2, 3, 6, 7)
-// Ghost lanes work in a ROTATED frame (normal, tangential, z): only shared-memory offsets differ between the lanes.
+// All ten warps run ONE instruction stream with the same arithmetic (a ghost column is predicted exactly like an
+// interior one, so data uniform along an axis stay bit-identically uniform); the roles differ in a few warp-uniform
+// branches and in which states a lane publishes or keeps.
 // Per slot s (plane pair s of the flat sequence; everything a neighbour publishes is double-buffered):
 //   C  cons -> prim of pair s+1 (raw pairs arrive by TMA: box 20 x 20 x 2 x 5, ring of ZNS stages) -> W[(s+1)&1]
 //   P  slopes, face values, own-direction fluxes -> dU, the six predicted states, guard (reading R7);
@@ -205,20 +207,11 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   }
   const int w_own = 2 * ((j + 2) * ZWP + (i + 2));          // float offsets (8-byte elements)
   const int raw_own = (j + 2) * FS + (i + 2);
-  // neighbour strides and the component planes holding the normal / tangential velocity (float offsets)
-  const int offn = rot ? 2 * ZWP : 2;
-  const int offt = rot ? 2 : 2 * ZWP;
-  const int cq1 = rot ? 4 * ZWQ : 2 * ZWQ;
-  const int cq2 = rot ? 2 * ZWQ : 4 * ZWQ;
-  auto wq = [&](int q) { return q == 1 ? cq1 : (q == 2 ? cq2 : 2 * q * ZWQ); };
   // exchange arrays of one pair: [SX: 6 x ZNX][SY: 6 x ZNY] and [FX: 5 x ZNX][FY: 5 x ZNY], 8-byte elements
   const int ix = 2 * (i + 17 * j), iy = 2 * (i + 16 * j);   // own lower x / y face (float offsets)
-  // where the '+' state along the first direction is published: x+ of cell (i, j) -> SX[(i+1) + 17 j]; a rotated
-  // ghost lane's y+ -> SY[i + 16 (j+1)] with the slots of u and v exchanged
-  const bool p1y = rot;
-  const int p1o = rot ? iy + 2 * FN : ix + 2;
-  const int p1s = rot ? 2 * ZNY : 2 * ZNX;
-  const int p1u = rot ? 2 * p1s : p1s, p1v = rot ? p1s : 2 * p1s;
+  // who publishes which '+' state: x+ of cell (i, j) -> SX[(i+1) + 17 j] (interior and the ghost column i = -1),
+  // y+ -> SY[i + 16 (j+1)] (interior and the ghost row j = -1)
+  const bool pub_x = role == 0 || (role == 2 && !rot), pub_y = role == 0 || (role == 2 && rot);
 
   const int n_local = (n_groups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;
   const int n_slots = n_local * ZSLOTS;
@@ -263,7 +256,7 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   };
   auto load_own = [&](const float* wpl, f2 W[5]) {   // own column of a primitive pair-plane, rotated frame
 #pragma unroll
-    for (int q = 0; q < 5; ++q) W[q] = lds2(wpl + w_own + wq(q));
+    for (int q = 0; q < 5; ++q) W[q] = lds2(wpl + w_own + 2 * q * ZWQ);
   };
 
   unsigned int n_guard = 0, n_nonpos = 0;
@@ -272,9 +265,8 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   {  // pair 0 of the flat sequence (planes -3, -2 of the first group)
     f2 W[5];
     convert(next_raw(), raw_own, W);
-    Wc[0] = W[0]; Wc[3] = W[3]; Wc[4] = W[4];
-    Wc[1] = rot ? W[2] : W[1];
-    Wc[2] = rot ? W[1] : W[2];
+#pragma unroll
+    for (int q = 0; q < 5; ++q) Wc[q] = W[q];
 #pragma unroll
     for (int q = 0; q < 5; ++q) az[q] = 0.0f;
   }
@@ -316,24 +308,21 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
         for (int q = 0; q < 5; ++q) sts2(we + 2 * q * ZWQ, We[q]);
       }
     }
-    const float n1 = rot ? lo(Wn[2]) : lo(Wn[1]);
-    const float n2 = rot ? lo(Wn[1]) : lo(Wn[2]);
-    cz[0] = lo(Wn[0]) - hi(Wc[0]); cz[1] = n1 - hi(Wc[1]); cz[2] = n2 - hi(Wc[2]);
-    cz[3] = lo(Wn[3]) - hi(Wc[3]); cz[4] = lo(Wn[4]) - hi(Wc[4]);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) cz[q] = lo(Wn[q]) - hi(Wc[q]);
   };
 
   // ---- P: reconstruction + half-step prediction of the pair; publishes the x+ / y+ states into S[buf]
   // Sm1, Sm2: the '-' states along the two in-plane directions (interior: x-, y-; upper ghosts use Sm1); Szm, Szp: z-, z+
   auto phaseP = [&](const float* w_cur, float* sx, float* sy, const float cz[5], St2& Sm1, St2& Sm2, St2& Szm, St2& Szp) {
-    float* const p1 = (p1y ? sy : sx) + p1o;
     f2 s1[5], s2[5], s3[5];
     {
       const float* wp = w_cur + w_own;
 #pragma unroll
       for (int q = 0; q < 5; ++q) {
-        const int o = wq(q);
-        const f2 a1 = Wc[q] - lds2(wp + o - offn), b1 = lds2(wp + o + offn) - Wc[q];
-        const f2 a2 = Wc[q] - lds2(wp + o - offt), b2 = lds2(wp + o + offt) - Wc[q];
+        const int o = 2 * q * ZWQ;
+        const f2 a1 = Wc[q] - lds2(wp + o - 2), b1 = lds2(wp + o + 2) - Wc[q];
+        const f2 a2 = Wc[q] - lds2(wp + o - 2 * ZWP), b2 = lds2(wp + o + 2 * ZWP) - Wc[q];
         s1[q] = limited_slope2<LIM>(a1, b1);
         s2[q] = limited_slope2<LIM>(a2, b2);
         const float bz = hi(Wc[q]) - lo(Wc[q]);
@@ -350,19 +339,19 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
       for (int q = 0; q < 5; ++q) dU[q] = c.hlamn * acc[q];
     }
     f2 gmin = c.one;
-    // '+' states along the first / second in-plane direction: published where a neighbour needs them — interior: x+ ->
-    // SX[(i+1) + 17 j], y+ -> SY[i + 16 (j+1)]; lower ghosts: the normal one -> SX[17 j] / SY[i], rotated slots
+    // x+ / y+ states: published where a neighbour needs them (the ghost columns run the very same arithmetic as the
+    // interior ones — no rotated frame — so that data uniform along an axis give bit-identical states along it)
     {
       const St2 S = zp_state<+1>(U1p, dU, c, gmin);
-      if (role != 1) {
-        float* o = p1;
-        sts2(o, S.r); sts2(o + p1u, S.u); sts2(o + p1v, S.v); sts2(o + 3 * p1s, S.w);
-        sts2(o + 4 * p1s, S.p); sts2(o + 5 * p1s, S.h);
+      if (pub_x) {
+        float* o = sx + ix + 2;
+        sts2(o, S.r); sts2(o + 2 * ZNX, S.u); sts2(o + 4 * ZNX, S.v); sts2(o + 6 * ZNX, S.w);
+        sts2(o + 8 * ZNX, S.p); sts2(o + 10 * ZNX, S.h);
       }
     }
     {
       const St2 S = zp_state<+1>(U2p, dU, c, gmin);
-      if (role == 0) {
+      if (pub_y) {
         float* o = sy + iy + 2 * FN;
         sts2(o, S.r); sts2(o + 2 * ZNY, S.u); sts2(o + 4 * ZNY, S.v); sts2(o + 6 * ZNY, S.w);
         sts2(o + 8 * ZNY, S.p); sts2(o + 10 * ZNY, S.h);
@@ -387,15 +376,15 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
       fix_state(Szm, ok_lo, ok_hi, fb); fix_state(Szp, ok_lo, ok_hi, fb);
       const float fl[6] = {lo(fb.r), lo(fb.u), lo(fb.v), lo(fb.w), lo(fb.p), lo(fb.h)};
       const float fh[6] = {hi(fb.r), hi(fb.u), hi(fb.v), hi(fb.w), hi(fb.p), hi(fb.h)};
-      const int so[6] = {0, p1u, p1v, 3 * p1s, 4 * p1s, 5 * p1s};
+      float* ox = sx + ix + 2;
       float* oy = sy + iy + 2 * FN;
 #pragma unroll
       for (int m = 0; m < 6; ++m) {
-        if (role != 1) {
-          if (!ok_lo) p1[so[m]] = fl[m];
-          if (!ok_hi) p1[so[m] + 1] = fh[m];
+        if (pub_x) {
+          if (!ok_lo) ox[2 * m * ZNX] = fl[m];
+          if (!ok_hi) ox[2 * m * ZNX + 1] = fh[m];
         }
-        if (role == 0) {
+        if (pub_y) {
           if (!ok_lo) oy[2 * m * ZNY] = fl[m];
           if (!ok_hi) oy[2 * m * ZNY + 1] = fh[m];
         }
@@ -487,17 +476,21 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
         accxy[q] = Fx[q] + Fy[q];
       }
     } else if (role == 1) {
-      // the face this ghost owns: x = 15.5 (column i = 16) or y = 15.5 (row j = 16), solved in the rotated frame
+      // the face this ghost owns: x = 15.5 (column i = 16: left state SX[16 + 17 j], right state its x- state) or
+      // y = 15.5 (row j = 16: SY[i + 256], its y- state). The row lanes feed the solver their velocities in the cyclic
+      // order (v, w, u) of the interior's y solve, so that both perform the same operations on the same operands
       const float* p = rot ? (sy + iy) : (sx + ix);
       const int st = rot ? 2 * ZNY : 2 * ZNX;
-      const int s1o = rot ? 2 * st : st, s2o = rot ? st : 2 * st;
-      St2 Lq;
-      Lq.r = lds2(p); Lq.u = lds2(p + s1o); Lq.v = lds2(p + s2o); Lq.w = lds2(p + 3 * st);
+      const int o1 = rot ? 2 * st : st, o2 = rot ? 3 * st : 2 * st, o3 = rot ? st : 3 * st;   // slots of (normal, t1, t2)
+      St2 Lq, Rq;
+      Lq.r = lds2(p); Lq.u = lds2(p + o1); Lq.v = lds2(p + o2); Lq.w = lds2(p + o3);
       Lq.p = lds2(p + 4 * st); Lq.h = lds2(p + 5 * st);
+      Rq.r.v = rot ? Sm2.r.v : Sm1.r.v; Rq.p.v = rot ? Sm2.p.v : Sm1.p.v; Rq.h.v = rot ? Sm2.h.v : Sm1.h.v;
+      Rq.u.v = rot ? Sm2.v.v : Sm1.u.v; Rq.v.v = rot ? Sm2.w.v : Sm1.v.v; Rq.w.v = rot ? Sm2.u.v : Sm1.w.v;
       f2 F[5];
-      roe2<0>(Lq, Sm1, c, F);
+      roe2<0>(Lq, Rq, c, F);
       float* o = rot ? (fy + iy) : (fx + ix);
-      sts2(o, F[0]); sts2(o + s1o, F[1]); sts2(o + s2o, F[2]); sts2(o + 3 * st, F[3]); sts2(o + 4 * st, F[4]);
+      sts2(o, F[0]); sts2(o + o1, F[1]); sts2(o + o2, F[2]); sts2(o + o3, F[3]); sts2(o + 4 * st, F[4]);
     }
   };
 
@@ -530,7 +523,7 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
     if (duty) {
       if (ZROT && role != 0) {
         az[0] = w_nxt[w_own + 1];   // upper plane of pair s-1 (this warp's pair-plane of two slots ago, about to be overwritten)
-        az[1] = w_nxt[w_own + cq1 + 1]; az[2] = w_nxt[w_own + cq2 + 1];
+        az[1] = w_nxt[w_own + 2 * ZWQ + 1]; az[2] = w_nxt[w_own + 4 * ZWQ + 1];
         az[3] = w_nxt[w_own + 6 * ZWQ + 1]; az[4] = w_nxt[w_own + 8 * ZWQ + 1];
         load_own(w_cur, Wc);
 #pragma unroll

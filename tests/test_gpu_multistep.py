@@ -65,8 +65,11 @@ def test_max_speed_matches_the_fp64_formula():
     assert gh.gamer_hydro_max_speed(torch.from_numpy(poisoned).to(DEV)) == got
 
 
+@pytest.mark.parametrize("path", [gh.PATH_AUTO, gh.PATH_FUSED_DUO])
 @pytest.mark.parametrize("cfg", ["turbulence", "sod_tube"])
-def test_device_resident_advance_matches_host_driven_steps_and_the_oracle(cfg):
+def test_device_resident_advance_matches_host_driven_steps_and_the_oracle(cfg, path):
+    """gamer_hydro_advance on the default path (step + ghost refill) and on the DUO path (on a periodic grid: the
+    fused-halo step kernel) against host-driven steps through the same kernel path (bit-identical) and the oracle."""
     if cfg == "turbulence":
         w, steps = wl.config_2_turbulence(64, seed=2, steps=10), 10
     else:
@@ -77,15 +80,19 @@ def test_device_resident_advance_matches_host_driven_steps_and_the_oracle(cfg):
     n = d_U.shape[0]
     d_out = torch.empty((n, 5, 16, 16, 16), dtype=torch.float32, device=DEV)
     d_bf = torch.empty((n, 6, 5, 16, 16), dtype=torch.float32, device=DEV)
-    dts = gh.gamer_hydro_advance(d_U, d_out, d_bf, grid, steps, w.cfl, dx, bc=bc, limiter=w.limiter)
-    torch.cuda.synchronize()
+    gh.gamer_hydro_set_path(path)
+    try:
+        dts = gh.gamer_hydro_advance(d_U, d_out, d_bf, grid, steps, w.cfl, dx, bc=bc, limiter=w.limiter)
+        torch.cuda.synchronize()
+    finally:
+        gh.gamer_hydro_set_path(gh.PATH_AUTO)
     assert len(dts) == steps and all(dt > 0 for dt in dts)
     # the harness' fp64 time step on the initial box agrees with the device's first one
     assert abs(dts[0] - wl.cfl_dt(w.U, w.dx, w.cfl)) <= 2e-6 * dts[0]
     # (1) host-driven loop through the plain step call with the same dt sequence: bit-identical
     U = w.U.copy()
     for dt in dts:
-        out = pu.run_gpu(wl.cut_groups(U, w.bc), dt, dx, G, w.limiter, want_bflux=False)[0]
+        out = pu.run_gpu(wl.cut_groups(U, w.bc), dt, dx, G, w.limiter, want_bflux=False, path=path)[0]
         U = wl.assemble_box(out, w.shape)
     assert np.array_equal(d_out.cpu().numpy(), out)
     assert np.array_equal(d_U.cpu().numpy(), wl.cut_groups(U, w.bc))       # ghost shells refilled for the next step
@@ -138,7 +145,11 @@ def test_fused_halo_step_equals_step_plus_ghost_refill(shape, limiter):
         if fused:
             gh.gamer_hydro_step_grid(d_in, d_out, d_bf, d_next, grid, dt, dx, limiter=limiter)
         else:
-            gh.gamer_hydro_step(d_in, d_out, d_bf, n, 16, 2, dt, dx, G, limiter)
+            gh.gamer_hydro_set_path(gh.PATH_FUSED_DUO)      # the fused-halo kernel is the DUO kernel with HALO = true
+            try:
+                gh.gamer_hydro_step(d_in, d_out, d_bf, n, 16, 2, dt, dx, G, limiter)
+            finally:
+                gh.gamer_hydro_set_path(gh.PATH_AUTO)
             gh.gamer_hydro_fill_ghosts(d_out, d_next, grid)
         torch.cuda.synchronize()
         outs.append((d_out.cpu().numpy(), d_bf.cpu().numpy(), d_next.cpu().numpy()))
@@ -151,9 +162,10 @@ def test_fused_halo_step_equals_step_plus_ghost_refill(shape, limiter):
         gh.gamer_hydro_step_grid(d_in, d_out, d_bf, d_in, grid, dt, dx)        # U_next aliases the input
 
 
-def test_advance_odd_and_even_step_counts_on_a_periodic_grid():
-    """The fused-halo loop ping-pongs between the caller's array and the library's: the caller's array must hold the
-    final ghosted state for odd and even step counts alike."""
+@pytest.mark.parametrize("path", [gh.PATH_AUTO, gh.PATH_FUSED_DUO])
+def test_advance_odd_and_even_step_counts_on_a_periodic_grid(path):
+    """The fused-halo loop (DUO path) ping-pongs between the caller's array and the library's: the caller's array must
+    hold the final ghosted state for odd and even step counts alike; the default path refills in place."""
     w = wl.config_2_turbulence(32, seed=7)
     grid, bc = _grid(w.shape), [BC[b] for b in w.bc]
     dx = pu.f32(w.dx)
@@ -161,11 +173,15 @@ def test_advance_odd_and_even_step_counts_on_a_periodic_grid():
         d_U = torch.from_numpy(w.groups()).to(DEV)
         n = d_U.shape[0]
         d_out = torch.empty((n, 5, 16, 16, 16), dtype=torch.float32, device=DEV)
-        dts = gh.gamer_hydro_advance(d_U, d_out, None, grid, steps, w.cfl, dx, bc=bc, limiter=w.limiter)
-        torch.cuda.synchronize()
+        gh.gamer_hydro_set_path(path)
+        try:
+            dts = gh.gamer_hydro_advance(d_U, d_out, None, grid, steps, w.cfl, dx, bc=bc, limiter=w.limiter)
+            torch.cuda.synchronize()
+        finally:
+            gh.gamer_hydro_set_path(gh.PATH_AUTO)
         U = w.U.copy()
         for dt in dts:
-            out = pu.run_gpu(wl.cut_groups(U, w.bc), dt, dx, G, w.limiter, want_bflux=False)[0]
+            out = pu.run_gpu(wl.cut_groups(U, w.bc), dt, dx, G, w.limiter, want_bflux=False, path=path)[0]
             U = wl.assemble_box(out, w.shape)
         assert np.array_equal(d_out.cpu().numpy(), out)
         assert np.array_equal(d_U.cpu().numpy(), wl.cut_groups(U, w.bc)), steps
@@ -186,15 +202,23 @@ def test_fused_halo_step_on_the_guard_heavy_cosmo_field():
         if fused:
             gh.gamer_hydro_step_grid(d_in, d_out, None, d_next, grid, dt, dx, limiter=w.limiter)
         else:
-            gh.gamer_hydro_step(d_in, d_out, None, n, 16, 2, dt, dx, G, w.limiter)
+            gh.gamer_hydro_set_path(gh.PATH_FUSED_DUO)
+            try:
+                gh.gamer_hydro_step(d_in, d_out, None, n, 16, 2, dt, dx, G, w.limiter)
+            finally:
+                gh.gamer_hydro_set_path(gh.PATH_AUTO)
             gh.gamer_hydro_fill_ghosts(d_out, d_next, grid)
         torch.cuda.synchronize()
         res.append((d_out.cpu().numpy(), d_next.cpu().numpy(), gh.gamer_hydro_status()))
     assert res[0][2] == res[1][2] and res[0][2][0] > 0          # same guard / non-positive counts, guard active
     assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
     # the signal-speed maximum the fused kernel leaves for the next step is the maximum of the new state
-    dts = gh.gamer_hydro_advance(torch.from_numpy(grp).to(DEV), torch.empty((n, 5, 16, 16, 16), device=DEV), None, grid, 2,
-                                 0.5, dx, limiter=w.limiter)
+    gh.gamer_hydro_set_path(gh.PATH_FUSED_DUO)
+    try:
+        dts = gh.gamer_hydro_advance(torch.from_numpy(grp).to(DEV), torch.empty((n, 5, 16, 16, 16), device=DEV), None,
+                                     grid, 2, 0.5, dx, limiter=w.limiter)
+    finally:
+        gh.gamer_hydro_set_path(gh.PATH_AUTO)
     vnew = gh.gamer_hydro_max_speed(torch.from_numpy(res[1][0]).to(DEV), ghost=0)
     # (advance's first step used its own dt, so only check the relation dt = cfl dx / vmax on the second step loosely)
     assert dts[1] > 0 and np.isfinite(vnew)
