@@ -5,8 +5,11 @@ One "step" = one pass of the whole hot path (reconstruction, half-step predictio
 update, boundary fluxes) over one batch of synthetic patch groups. At N = 1 the workload is
 BASELINE.json:configs[3], the configuration the metric is quoted on: 32768 groups of 16^3 cells (+2 ghost
 layers) cut from a seeded 512^3 cosmology-like baryonic field, fp32, gamma = 5/3, MinMod, one step per
-launch. With N > 1 (torchrun, one rank per GPU) every rank owns its own 32768-group batch (seed + rank):
-patch groups are independent, so the path shards with no collective ("scaling": "weak").
+launch. With N > 1 there is one rank per GPU (`python bench.py --gpus N` re-executes itself under
+torch.distributed.run when it was not started by it); patch groups are independent, so the path shards with no
+collective: `--scaling weak` (default) gives every rank the full 32768-group batch, `--scaling strong` splits the ONE
+batch into contiguous group ranges (paper_1007_3818_b200/sharding.py). The field is generated once (rank 0) and
+shared with the other ranks through a file in /dev/shm.
 
 Contract: `python bench.py --gpus N --steps K --warmup W [--impl reference]` prints ONE JSON line on rank 0.
   value      whole-job cell-updates/s with inputs resident in HBM (CUDA events, max over ranks)
@@ -36,6 +39,7 @@ N, GHOST = 16, 2
 # algorithmic FLOPs per cell-update: oracle CountingReal tally on an all-slopes-active field (
 # tests/test_oracle_pins.py::test_flop_tally_band re-derives it). Hand count of SURVEY.md App. D: 925 / 966.
 FLOPS_PER_CELL = {0: 1033.94, 1: 1095.81}
+FLOPS_PER_CELL_HAND = {0: 925.0, 1: 966.0}
 BYTES_PER_CELL = 66.5625           # (5*20^3 + 5*16^3 + 30*16^2) * 4 B / 16^3
 SM_COUNT, LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = SM_COUNT * LANES * 2 * SM_MAX_GHZ / 1e3     # 74.45
@@ -97,7 +101,7 @@ class ClockSampler(threading.Thread):
 
 
 def make_workload(n_box, seed):
-    from paper_1007_3818_b200 import workloads as wl
+    from harness import workloads as wl
     t0 = time.time()
     w = wl.config_3_cosmo(n_box, seed=seed)
     groups = w.groups(np.float32)
@@ -133,6 +137,51 @@ def run_reference(args, rank, world):
         "gpu_launches": 0}))
 
 
+def maybe_respawn(args):
+    """`python bench.py --gpus N` with N > 1 and no torchrun environment: start N ranks of this script under
+    torch.distributed.run on this node (one GPU each) and exit with their status."""
+    if args.gpus <= 1 or "WORLD_SIZE" in os.environ:
+        return
+    import socket
+    import subprocess
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
+def shared_workload(args, rank, world, barrier):
+    """The cfg3 field, generated ONCE (rank 0) and shared with the other ranks of the node through /dev/shm."""
+    if world == 1:
+        return make_workload(args.box, args.seed)
+    from harness import workloads as wl
+    tag = "gamer_bench_%s_%d_%d" % (os.environ.get("MASTER_PORT", "0"), args.box, args.seed)
+    base = os.path.join("/dev/shm" if os.path.isdir("/dev/shm") else "/tmp", tag)
+    t0 = time.time()
+    if rank == 0:
+        w, groups, dt, dx, _ = make_workload(args.box, args.seed)
+        np.save(base + ".npy", groups)
+        with open(base + ".json", "w") as f:
+            json.dump({"dt": dt, "dx": dx}, f)
+    barrier()
+    if rank != 0:
+        w = wl.Workload("cfg3_cosmo_%d" % args.box, None, 1.0 / args.box, ("periodic",) * 3, 0, 0.5, 1)
+        groups = np.load(base + ".npy", mmap_mode="r")
+        with open(base + ".json") as f:
+            meta = json.load(f)
+        dt, dx = meta["dt"], meta["dx"]
+    barrier()
+    if rank == 0:
+        for ext in (".npy", ".json"):
+            try:
+                os.remove(base + ext)
+            except OSError:
+                pass
+    return w, groups, dt, dx, time.time() - t0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -141,6 +190,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--box", type=int, default=512, help="global box edge; 512 -> 32768 groups (headline)")
     ap.add_argument("--seed", type=int, default=3)
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = the full batch on every rank; strong = the one batch split by sharding.shard_range")
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-groups", type=int, default=4096,
                     help="groups in the oracle sample (cpu_baseline): 16.8 M cell-updates, about 15 core-seconds")
@@ -148,10 +199,14 @@ def main():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-multistep", action="store_true")
+    ap.add_argument("--no-cuda", action="store_true",
+                    help="launcher self-test (CPU, gloo): everything up to, not including, the first CUDA call")
     ap.add_argument("--path", default="auto", choices=["auto", "generic", "fused", "fused_scalar", "fused_duo"],
                     help="kernel path forced through gamer_hydro_set_path (default: the library's choice)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "ours":
+        maybe_respawn(args)
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
@@ -162,6 +217,28 @@ def main():
 
     import torch
     import torch.distributed as dist
+    from paper_1007_3818_b200 import sharding
+
+    if args.no_cuda:
+        # the N > 1 plumbing without a GPU: rendezvous, one field for all ranks, the partition, the timing reduction
+        if world > 1:
+            dist.init_process_group("gloo")
+        cpu_barrier = (lambda: dist.barrier()) if world > 1 else (lambda: None)
+        w, groups, dt, dx, gen_s = shared_workload(args, rank, world, cpu_barrier)
+        a, b = sharding.shard_range(groups.shape[0], rank, world) if args.scaling == "strong" else (0, groups.shape[0])
+        mine = np.ascontiguousarray(groups[a:b])
+        t = sharding.max_over_ranks(1.0 + rank)
+        counts = torch.tensor([b - a], dtype=torch.int64)
+        if world > 1:
+            dist.all_reduce(counts)
+        if rank == 0:
+            print(json.dumps({"launcher_self_test": True, "n_gpus": world, "scaling": args.scaling,
+                              "groups_total": int(counts.item()), "groups_rank0": int(mine.shape[0]),
+                              "max_over_ranks": t, "checksum_rank0": float(np.asarray(mine, dtype=np.float64).sum())}))
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
     import paper_1007_3818_b200 as gh
 
     if not torch.cuda.is_available():
@@ -171,7 +248,15 @@ def main():
     if world > 1:
         dist.init_process_group("nccl", device_id=dev)
 
-    w, groups, dt, dx, gen_s = make_workload(args.box, args.seed + rank)
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    w, all_groups, dt, dx, gen_s = shared_workload(args, rank, world, barrier)
+    g0, g1 = sharding.shard_range(all_groups.shape[0], rank, world) if args.scaling == "strong" else (0, all_groups.shape[0])
+    groups = np.ascontiguousarray(all_groups[g0:g1])
     G = groups.shape[0]
     cells = G * N ** 3
     gh.gamer_hydro_alloc(G, N, GHOST, 4, local_rank)
@@ -184,12 +269,6 @@ def main():
 
     def step():
         gh.gamer_hydro_step(d_in, d_out, d_bf, G, N, GHOST, dt, dx, w.gamma, w.limiter, stream=stream)
-
-    def barrier():
-        torch.cuda.synchronize()
-        if world > 1:
-            dist.barrier()
-            torch.cuda.synchronize()
 
     for _ in range(args.warmup):
         step()
@@ -210,11 +289,13 @@ def main():
     total_ms = evs[0].elapsed_time(evs[-1])
     per_step = [evs[s].elapsed_time(evs[s + 1]) for s in range(args.steps)]
     guard_cells, nonpos = gh.gamer_hydro_status()
-    tmax = torch.tensor([total_ms], dtype=torch.float64, device=dev)
+    total_ms_max = sharding.max_over_ranks(total_ms, device=dev)          # the slowest rank sets the job's time
+    cells_all = cells
     if world > 1:
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    total_ms_max = float(tmax.item())
-    value = world * cells * args.steps / (total_ms_max * 1e-3)
+        ct = torch.tensor([cells], dtype=torch.int64, device=dev)
+        dist.all_reduce(ct)
+        cells_all = int(ct.item())
+    value = cells_all * args.steps / (total_ms_max * 1e-3)                # == sharding.aggregate_throughput for equal shards
 
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
     e2e = None
@@ -232,15 +313,30 @@ def main():
         for _ in range(args.e2e_steps):
             e2e_step()
         barrier()
-        te = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(te, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * cells * args.e2e_steps / float(te.item()), "unit": UNIT,
-               "h2d_bytes_per_step": int(hp_in.numel() * 4),
-               "d2h_bytes_per_step": int((hp_out.numel() + hp_bf.numel()) * 4),
-               "steps": args.e2e_steps, "api": "gamer_hydro_step_host (pinned host buffers, chunked 3-stream overlap)"}
-        same = bool(torch.equal(hp_out, d_out.cpu()))
-        e2e["matches_device_path_bitwise"] = same
+        te = sharding.max_over_ranks(time.perf_counter() - t0, device=dev)
+        h2d_b, d2h_b = int(hp_in.numel() * 4), int((hp_out.numel() + hp_bf.numel()) * 4)
+        # the host link's own speed, measured in the same run: one pinned H2D copy of the input, one D2H of the output
+        c0, c1, c2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+        d_in.copy_(hp_in, non_blocking=True)
+        barrier()
+        c0.record(stream)
+        d_in.copy_(hp_in, non_blocking=True)
+        c1.record(stream)
+        hp_out.copy_(d_out, non_blocking=True)
+        c2.record(stream)
+        barrier()
+        h2d_peak = h2d_b / (c0.elapsed_time(c1) * 1e-3) / 1e9
+        d2h_peak = hp_out.numel() * 4 / (c1.elapsed_time(c2) * 1e-3) / 1e9
+        t_step = te / args.e2e_steps
+        # H2D and D2H run on different copy engines and overlap: the link-bound time of a step is the longer of the two
+        t_link = max(h2d_b / (h2d_peak * 1e9), d2h_b / (d2h_peak * 1e9))
+        e2e = {"value": cells_all * args.e2e_steps / te, "unit": UNIT,
+               "h2d_bytes_per_step": h2d_b, "d2h_bytes_per_step": d2h_b, "steps": args.e2e_steps,
+               "api": "gamer_hydro_step_host (pinned host buffers, chunked 3-stream overlap)",
+               "h2d_gbs_achieved": h2d_b / t_step / 1e9, "d2h_gbs_achieved": d2h_b / t_step / 1e9,
+               "h2d_gbs_pinned_copy_alone": h2d_peak, "d2h_gbs_pinned_copy_alone": d2h_peak,
+               "frac_of_link_bound_time": t_link / t_step}
+        e2e["matches_device_path_bitwise"] = bool(torch.equal(hp_out, d_out.cpu()))
         del hp_in, hp_out, hp_bf
 
     if rank != 0:
@@ -248,27 +344,32 @@ def main():
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the dominant (only) kernel of the step (pair_kernel<MinMod> on the default path)
+    # ---- roofline of the dominant (only) kernel of the step
     ms_launch = total_ms / args.steps                         # one launch per step on this rank
     flops = FLOPS_PER_CELL[w.limiter] * cells
     achieved_tf = flops / (ms_launch * 1e-3) / 1e12
     hbm_peak, hbm_src = measured_hbm_peak()
     hbm_gbs = BYTES_PER_CELL * cells / (ms_launch * 1e-3) / 1e9
-    traffic = None
+    traffic, traffic_src = None, None
     try:
-        with open(os.path.join(ROOT, "profiles", "r1d_traffic_bytes_per_launch.txt")) as f:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic_bytes_per_launch.txt")) as f:
             tj = json.load(f)
-            if tj.get("n_groups") == G:
+            if tj.get("n_groups") == G and args.path in ("auto", "fused"):
                 traffic = tj["dram_bytes_read_plus_write"]
+                traffic_src = "ncu --set full capture, profiles/r2_traffic_bytes_per_launch.txt (commit %s)" % tj.get("commit")
     except Exception:
         pass
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
-                "frac": achieved_tf / ALU_PEAK_TFLOPS, "traffic": traffic,
-                "kernel": {"auto": "gh::duo_kernel<MinMod>", "fused": "gh::duo_kernel<MinMod>",
+                "frac": achieved_tf / ALU_PEAK_TFLOPS, "traffic": traffic, "traffic_source": traffic_src,
+                "kernel": {"auto": "gh::zpair_kernel<MinMod>", "fused": "gh::zpair_kernel<MinMod>",
                            "fused_scalar": "gh::fused_kernel<float, MinMod, fast>",
-                           "fused_pair": "gh::pair_kernel<MinMod>",
+                           "fused_duo": "gh::duo_kernel<MinMod>",
                            "generic": "gh::predict_kernel + flux_kernel + update_kernel"}[args.path],
                 "flops_per_cell_update": FLOPS_PER_CELL[w.limiter],
+                "flops_source": "oracle CountingReal tally (DESIGN.md section 6); SURVEY.md App. D hand count: %g"
+                                % FLOPS_PER_CELL_HAND[w.limiter],
+                "frac_with_hand_count": FLOPS_PER_CELL_HAND[w.limiter] * cells / (ms_launch * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                "target_frac": 0.60, "target_met": bool(achieved_tf / ALU_PEAK_TFLOPS >= 0.60),
                 "peak_derivation": "148 SM x 128 FP32 lanes x 2 FLOP x 1.965 GHz (sm_max_mhz of MEASURED_PEAKS.json)",
                 "ms_per_launch": ms_launch,
                 "hbm": {"algorithmic_bytes_per_launch": BYTES_PER_CELL * cells, "achieved_gbs": hbm_gbs,
@@ -280,9 +381,7 @@ def main():
     cpu = None
     if not args.no_cpu_baseline and world == 1:
         from oracle import mhm_oracle as O
-        sys.path.insert(0, os.path.join(ROOT, "tests"))
-        import metrics
-        import parity_util as pu
+        from harness import metrics
         rng = np.random.default_rng(12345)
         rho_max = groups[:, 0, 2:-2, 2:-2, 2:-2].reshape(G, -1).max(axis=1)
         pick = set(int(i) for i in rng.choice(G, size=min(args.cpu_groups, G) - 2, replace=False))
@@ -292,12 +391,18 @@ def main():
         t0 = time.perf_counter()
         r = O.step_groups(sample, N, GHOST, dt, dx, w.gamma, w.limiter)
         tc = time.perf_counter() - t0
+        n1 = min(256, len(idx))                               # one thread: a smaller sample of the same groups
+        t0 = time.perf_counter()
+        O.step_groups(sample[:n1], N, GHOST, dt, dx, w.gamma, w.limiter, n_threads=1)
+        t1 = time.perf_counter() - t0
         gout = d_out[torch.from_numpy(idx).to(dev)].cpu().numpy()
-        sus = pu.suspect_mask(r.margin)
+        sus = metrics.suspect_mask(r.margin)
         err = metrics.max_rel_err(gout, r.U_out, w.gamma, mask=np.broadcast_to(~sus[:, None], r.U_out.shape))
         desc = "%d of the %d groups (seeded random + the groups holding max/min density), one step" % (len(idx), G)
         cpu = {"value": len(idx) * N ** 3 / tc, "unit": UNIT, "cores": r.threads, "kind": "oracle", "sample": desc,
-               "seconds": tc, "parity_max_rel_err_on_sample": err, "parity_tolerance": 1e-4,
+               "seconds": tc, "one_thread": {"value": n1 * N ** 3 / t1, "unit": UNIT, "cores": 1, "seconds": t1,
+                                             "sample": "the first %d groups of the same sample" % n1},
+               "parity_max_rel_err_on_sample": err, "parity_tolerance": 1e-4,
                "parity_excluded_fraction": float(sus.mean()), "oracle_guard_cells_on_sample": r.guard_cells}
 
     # ---- device-resident multi-step run on the same grid: signal-speed maximum + step + ghost
@@ -317,20 +422,22 @@ def main():
         torch.cuda.synchronize()
         ms_ms = e0.elapsed_time(e1) / nms
         multistep = {"value": cells / (ms_ms * 1e-3), "unit": UNIT, "steps": nms, "ms_per_step": ms_ms,
-                     "api": "gamer_hydro_advance on the periodic grid (per step: one kernel = step + halo written into the next "
-                            "ghosted array + signal-speed maximum; one 4-byte D2H read)",
+                     "api": "gamer_hydro_advance on the periodic grid (per step: the step kernel, the ghost-refill kernel "
+                            "that also accumulates the next signal-speed maximum, one 4-byte D2H read)",
                      "dt_first": ms_dts[0], "dt_last": ms_dts[-1]}
         del d_state
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
-           "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+           "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
            "config": {"workload": "cfg3_cosmo_%d (BASELINE.json:configs[3]): %d patch groups/GPU, 16^3+2 ghost, "
                                   "5 vars, gamma=5/3, MinMod, 1 step per launch" % (args.box, G),
-                      "groups_per_gpu": G, "cells_per_gpu": cells, "seed": args.seed,
+                      "groups_per_gpu": G, "cells_per_gpu": cells, "cells_all_gpus": cells_all, "seed": args.seed,
                       "l2": "inputs (%.2f GB/step) far larger than the 126 MB L2; no flush needed" %
                             (h_in.numel() * 4 / 1e9),
-                      "parallelism": "groups sharded across ranks, no collective",
+                      "parallelism": "groups sharded across ranks (%s), no collective" %
+                                     ("the one batch split into contiguous ranges" if args.scaling == "strong" and world > 1
+                                      else "the full batch on every rank"),
                       "generation_seconds": gen_s, "dt": dt, "dx": dx, "kernel_path": args.path},
            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "multistep": multistep,
            "gpu_launches": int(launches),

@@ -50,3 +50,18 @@ def bflux_errors(gb, ob, U_out_o, gamma):
             err[:, f, q] = np.abs(gb[:, f, q] - ob[:, f, q]) / sc[q]
     del adj
     return err
+
+
+NEAR_GUARD = 1e-5        # |internal/total energy| of the worst predicted face state below which fp32 may flip R7
+
+
+def suspect_mask(margin, N=16):
+    """Interior cells whose update can be touched by an fp32/fp64 disagreement on the R7 guard: cells whose
+    own or a face neighbour's guard margin (an array the reference side provides, [G,N+2,N+2,N+2]) is within
+    NEAR_GUARD of zero. Pure array logic: no method arithmetic."""
+    near = np.abs(margin) < NEAR_GUARD          # NaN (cells outside R) compares False
+    m = near.copy()
+    m[:, 1:] |= near[:, :-1]; m[:, :-1] |= near[:, 1:]
+    m[:, :, 1:] |= near[:, :, :-1]; m[:, :, :-1] |= near[:, :, 1:]
+    m[:, :, :, 1:] |= near[:, :, :, :-1]; m[:, :, :, :-1] |= near[:, :, :, 1:]
+    return m[:, 1:-1, 1:-1, 1:-1]

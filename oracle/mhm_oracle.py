@@ -1,6 +1,6 @@
 """oracle/mhm_oracle.py — ctypes face of the fp64 CPU oracle. TEST INFRASTRUCTURE, NOT PRODUCT CODE.
 
-Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import this.
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs (and tests/parity_util.py) may import this.
 It imports nothing from paper_1007_3818_b200 (the CUDA path) and never will. The arithmetic lives in
 oracle/mhm_oracle.hpp, which cites the passages it follows (SURVEY.md §8(c) O0–O8).
 

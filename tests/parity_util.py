@@ -1,15 +1,16 @@
 """Shared helpers of the GPU parity tests: run the oracle and the CUDA path on the same seeded float32
-inputs and compare element by element with the R14 metric (tests/metrics.py), with the guard-disagreement
+inputs and compare element by element with the R14 metric (harness/metrics.py), with the guard-disagreement
 accounting of reading R7."""
 import numpy as np
 import torch
 
-import metrics
+from harness import metrics
 import paper_1007_3818_b200 as gh
 from oracle import mhm_oracle as O
 
-NEAR_GUARD = 1e-5        # |internal/total energy| of the worst predicted face state below which fp32 may flip R7
+NEAR_GUARD = metrics.NEAR_GUARD
 MAX_EXCLUDED_FRACTION = 1e-5
+suspect_mask = metrics.suspect_mask
 
 
 def f32(x):
@@ -33,17 +34,6 @@ def run_gpu(groups, dt, dx, gamma, limiter, path=gh.PATH_AUTO, want_bflux=True, 
         gh.gamer_hydro_set_path(gh.PATH_AUTO)
     st = gh.gamer_hydro_status()
     return out.cpu().numpy(), (bf.cpu().numpy() if want_bflux else None), st
-
-
-def suspect_mask(margin, N=16):
-    """Interior cells whose update can be touched by an fp32/fp64 disagreement on the R7 guard: cells whose
-    own or a face neighbour's guard margin is within NEAR_GUARD of zero. margin: [G,N+2,N+2,N+2]."""
-    near = np.abs(margin) < NEAR_GUARD          # NaN (cells outside R) compares False
-    m = near.copy()
-    m[:, 1:] |= near[:, :-1]; m[:, :-1] |= near[:, 1:]
-    m[:, :, 1:] |= near[:, :, :-1]; m[:, :, :-1] |= near[:, :, 1:]
-    m[:, :, :, 1:] |= near[:, :, :, :-1]; m[:, :, :, :-1] |= near[:, :, :, 1:]
-    return m[:, 1:-1, 1:-1, 1:-1]
 
 
 def compare(groups, dt, dx, gamma, limiter, gpu_out, gpu_bf=None, N=16, ghost=2):

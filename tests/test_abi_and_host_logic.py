@@ -102,9 +102,9 @@ def test_product_never_imports_the_oracle_and_nothing_reads_work_dirs():
 
 
 def test_workloads_module_is_arithmetic_free_of_both_sides():
-    s = open(os.path.join(ROOT, "paper_1007_3818_b200", "workloads.py")).read()
+    s = open(os.path.join(ROOT, "harness", "workloads.py")).read()
     assert not re.search(r"^\s*(from|import)\s+\S*(torch|binding|oracle)", s, flags=re.M)
-    from paper_1007_3818_b200 import workloads as wl
+    from harness import workloads as wl
     g = wl.random_groups(2, seed=1)
     assert g.shape == (2, 5, 20, 20, 20) and g.dtype == np.float32
     assert np.array_equal(g, wl.random_groups(2, seed=1))          # reproducible from the seed alone

@@ -5,11 +5,11 @@ import numpy as np
 import pytest
 import torch
 
-import metrics
+from harness import metrics
 import parity_util as pu
 import paper_1007_3818_b200 as gh
 from oracle import mhm_oracle as O
-from paper_1007_3818_b200 import workloads as wl
+from harness import workloads as wl
 
 pytestmark = pytest.mark.gpu
 G = wl.GAMMA

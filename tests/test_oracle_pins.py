@@ -11,7 +11,7 @@ import pytest
 import exact_riemann as er
 import naive_mhm
 from oracle import mhm_oracle as O
-from paper_1007_3818_b200 import workloads as wl
+from harness import workloads as wl
 
 G = 5.0 / 3.0
 HERE = os.path.dirname(os.path.abspath(__file__))

@@ -12,7 +12,7 @@ import torch.multiprocessing as mp
 
 from oracle import mhm_oracle as O
 from paper_1007_3818_b200 import sharding
-from paper_1007_3818_b200 import workloads as wl
+from harness import workloads as wl
 
 
 def test_shard_range_partitions_every_batch():
@@ -63,3 +63,29 @@ def test_two_rank_gloo_shards_concatenate_to_the_unsharded_result(tmp_path):
     out = np.concatenate([np.load(tmp_path / ("out%d.npy" % r)) for r in range(world)])
     bf = np.concatenate([np.load(tmp_path / ("bf%d.npy" % r)) for r in range(world)])
     assert np.array_equal(out, full.U_out) and np.array_equal(bf, full.bflux)
+
+
+@pytest.mark.parametrize("scaling", ["weak", "strong"])
+def test_bench_launcher_spawns_its_ranks_and_shards_one_field(scaling):
+    """`python bench.py --gpus 2` must itself start two ranks (torch.distributed.run), share ONE generated field and
+    partition it with sharding.shard_range; --no-cuda runs that path on gloo up to, not including, the first CUDA call."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_PORT")}
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--no-cuda", "--box", "32",
+                          "--scaling", scaling], capture_output=True, text=True, env=env, timeout=300)
+    assert res.returncode == 0, res.stderr[-2000:]
+    line = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(line) == 1                                       # rank 0 alone prints
+    d = json.loads(line[0])
+    one = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--no-cuda", "--box", "32"],
+                         capture_output=True, text=True, env=env, timeout=300)
+    d1 = json.loads([l for l in one.stdout.splitlines() if l.startswith("{")][0])
+    assert d["n_gpus"] == 2 and d1["n_gpus"] == 1 and d["max_over_ranks"] == 2.0
+    if scaling == "strong":
+        assert d["groups_total"] == d1["groups_total"] == 8 and d["groups_rank0"] == 4
+    else:
+        assert d["groups_total"] == 16 and d["groups_rank0"] == 8
+        assert d["checksum_rank0"] == d1["checksum_rank0"]      # every rank holds the same, once-generated field
