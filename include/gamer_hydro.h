@@ -134,6 +134,13 @@ int gamer_hydro_advance(float* U_with_ghosts, float* U_out, float* boundary_flux
  * be NULL. */
 int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonpositive_out);
 
+/* Debug aid of the parity harness (R7: cells where GPU and oracle DISAGREE on the guard are excluded from
+ * the parity maximum). With device_map != NULL every later step call marks the cells whose predicted states fell
+ * back to first order: device_map[g][k+1][j+1][i+1] = 1, unsigned char [n_groups][N+2][N+2][N+2] in DEVICE memory,
+ * owned and zeroed by the caller, indices -1 .. N per axis (first ghost layer included). NULL (the default) switches
+ * it off. Process-global, synchronises the device; the map is written on the rare fallback path only. */
+int gamer_hydro_set_guard_map(unsigned char* device_map);
+
 /* Forces a kernel path (tests, benchmarking); GAMER_HYDRO_PATH_AUTO restores the default. */
 int gamer_hydro_set_path(int path);
 

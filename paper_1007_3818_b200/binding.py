@@ -20,7 +20,7 @@ PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_DUO = 0, 1, 2
 EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
            "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance",
-           "gamer_hydro_step_grid"]
+           "gamer_hydro_step_grid", "gamer_hydro_set_guard_map"]
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
@@ -48,6 +48,7 @@ def lib():
         L.gamer_hydro_fill_ghosts.argtypes = [vp, vp, i, i, i, i, i, i, i, i, i, vp]
         L.gamer_hydro_step_grid.argtypes = [vp, vp, vp, vp, i, i, i, i, i, f, f, f, i, vp]
         L.gamer_hydro_advance.argtypes = [vp, vp, vp, i, i, i, i, i, i, i, i, i, f, f, f, i, vp, vp]
+        L.gamer_hydro_set_guard_map.argtypes = [vp]
         L.gamer_hydro_launch_count.restype = C.c_ulonglong
         L.gamer_hydro_strerror.restype = C.c_char_p
         L.gamer_hydro_strerror.argtypes = [i]
@@ -198,6 +199,14 @@ def gamer_hydro_status():
 
 def gamer_hydro_set_path(path):
     _check(lib().gamer_hydro_set_path(int(path)))
+
+
+def gamer_hydro_set_guard_map(device_map):
+    """device_map: zeroed uint8 CUDA tensor [n_groups][N+2][N+2][N+2], or None to switch the export off."""
+    if device_map is not None and not (device_map.is_cuda and device_map.dtype == torch.uint8 and
+                                       device_map.is_contiguous()):
+        raise GamerHydroError("guard map must be a contiguous CUDA uint8 tensor")
+    _check(lib().gamer_hydro_set_guard_map(device_map.data_ptr() if device_map is not None else None))
 
 
 def gamer_hydro_launch_count():

@@ -263,8 +263,8 @@ int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int g
     R* bf = bflux ? bflux + (size_t)g0 * 30 * N * N : nullptr;
     const dim3 gp((unsigned)((ne + 127) / 128), ng), gf((unsigned)((nf + 127) / 128), ng),
         gu((unsigned)((nc + 127) / 128), ng);
-    if (limiter == 0) gh::predict_kernel<R, 0><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status);
-    else gh::predict_kernel<R, 1><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status);
+    if (limiter == 0) gh::predict_kernel<R, 0><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
+    else gh::predict_kernel<R, 1><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
     gh::flux_kernel<R><<<gf, 128, 0, stream>>>(FS, FL, bf, sh, c);
     gh::update_kernel<R><<<gu, 128, 0, stream>>>(in, FL, out, sh, c, g_state.status);
     g_launches.fetch_add(3);
@@ -572,6 +572,14 @@ int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonp
 int gamer_hydro_set_path(int path) {
   if (path < GAMER_HYDRO_PATH_AUTO || path > GAMER_HYDRO_PATH_FUSED_DUO) return GAMER_HYDRO_INVALID_ARG;
   g_state.path = path;
+  return 0;
+}
+
+int gamer_hydro_set_guard_map(unsigned char* device_map) {
+  int rc = ensure_init();
+  if (rc) return rc;
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpyToSymbol(gh::gh_guard_map, &device_map, sizeof(device_map)));
   return 0;
 }
 

@@ -380,6 +380,7 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
             ex_put(so, 3, SA.w); ex_put(so, 4, SA.p); ex_put(so, 5, SA.h);
           }
           n_guard += 1u;  // every cell that gets here is one whose states are used
+          mark_guard(g, FN, i, j, k);
         }
         zm = lane_lo(SC);
         zp = St1{hi(SC.r), hi(SC.v), hi(SC.u), hi(SC.w), hi(SC.p), hi(SC.h)};  // hi lane: slots (v, u, w)

@@ -230,6 +230,7 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         }
         const bool ok = predict_cell<R, LIM, Fast>(Wc, Wn_m, Wn_p, c, Wf);
         n_guard += ok ? 0u : 1u;
+        if (!ok) mark_guard(g, FN, i, j, k);
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
           xs[q * FNT + t] = Wf[0][1][q];

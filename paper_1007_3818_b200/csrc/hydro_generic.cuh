@@ -41,7 +41,8 @@ __device__ __forceinline__ void load_prim(const R* __restrict__ Ug, const Generi
 
 template <class R, int LIM>
 __global__ void __launch_bounds__(128) predict_kernel(const R* __restrict__ U_in, R* __restrict__ FS, GenericShape sh,
-                                                      GasConst<R> c, unsigned long long* __restrict__ status) {
+                                                      GasConst<R> c, unsigned long long* __restrict__ status,
+                                                      long long g0) {
   const int E = sh.E, N = sh.N;
   const long long e = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (e >= (long long)E * E * E) return;
@@ -56,7 +57,10 @@ __global__ void __launch_bounds__(128) predict_kernel(const R* __restrict__ U_in
   load_prim(Ug, sh, i, j, k - 1, c, Wm[2]); load_prim(Ug, sh, i, j, k + 1, c, Wp[2]);
   R Wf[3][2][5];
   const bool ok = predict_cell<R, LIM, false>(Wc, Wm, Wp, c, Wf);
-  if (!ok) atomicAdd(&status[0], 1ULL);
+  if (!ok) {
+    atomicAdd(&status[0], 1ULL);
+    mark_guard(g0 + blockIdx.y, N, i, j, k);
+  }
   R* out = FS + (long long)blockIdx.y * sh.fs_stride + e;
   const long long ev = (long long)E * E * E;
 #pragma unroll

@@ -9,6 +9,15 @@
 
 namespace gh {
 
+// Debug aid of the parity harness (gamer_hydro_set_guard_map, R7): when non-null, the kernels mark the cells
+// whose predicted states fell back to first order in map[g][k+1][j+1][i+1] (unsigned char, (N+2)^3 per group). Read on
+// the rare fallback path only.
+__device__ unsigned char* gh_guard_map = nullptr;
+__device__ __forceinline__ void mark_guard(long long g, int N, int i, int j, int k) {
+  unsigned char* m = gh_guard_map;
+  if (m) m[((g * (N + 2) + (k + 1)) * (N + 2) + (j + 1)) * (N + 2) + (i + 1)] = 1;
+}
+
 template <class R>
 struct GasConst {
   R gamma;      // ratio of specific heats

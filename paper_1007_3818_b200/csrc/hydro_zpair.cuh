@@ -390,6 +390,8 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
         }
       }
       n_guard += (ok_lo ? 0u : 1u) + (ok_hi ? 0u : 1u);   // every cell that gets here is one whose states are used
+      if (!ok_lo) mark_guard(g, FN, i, j, 2 * gs - 3);
+      if (!ok_hi) mark_guard(g, FN, i, j, 2 * gs - 2);
     }
   };
 

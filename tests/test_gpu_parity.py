@@ -18,9 +18,11 @@ PATHS = [gh.PATH_FUSED, gh.PATH_GENERIC, gh.PATH_FUSED_DUO, gh.PATH_FUSED_SCALAR
 
 
 def check(groups, dt, dx, limiter, path, tol, gamma=G, max_excl=pu.MAX_EXCLUDED_FRACTION, ghost=2):
-    out, bf, st = pu.run_gpu(groups, dt, dx, gamma, limiter, path=path, ghost=ghost)
+    gm = []
+    out, bf, st = pu.run_gpu(groups, dt, dx, gamma, limiter, path=path, ghost=ghost, guard_map=gm)
     assert np.isfinite(out).all() and np.isfinite(bf).all()
-    res = pu.compare(groups, dt, dx, gamma, limiter, out, bf, ghost=ghost)
+    res = pu.compare(groups, dt, dx, gamma, limiter, out, bf, ghost=ghost, gpu_guard=gm[0])
+    res["gpu_guard"] = gm[0]
     assert res["excluded_fraction"] <= max_excl, res["excluded_fraction"]
     assert res["err"] <= tol, res["err"]
     assert res["err_bflux"] <= 10 * tol, res["err_bflux"]
@@ -110,15 +112,20 @@ def test_cfg2_turbulence_1_and_10_steps(path):
 def test_cfg3_cosmo_small_with_guard_accounting(path):
     w = wl.config_3_cosmo(64, seed=3)
     grp = w.groups()
-    res, st = check(grp, w.dt(), pu.f32(w.dx), w.limiter, path, TOL32_1, max_excl=1e-3)
+    # cells where GPU and oracle disagree on the guard, with their face neighbours: at most 1e-4 of this small box
+    # (the Mach-30 cells are a far larger share of 64^3 than of the 512^3 headline box, which is held to R7's 1e-5)
+    res, st = check(grp, w.dt(), pu.f32(w.dx), w.limiter, path, TOL32_1, max_excl=1e-4)
     o = res["oracle"]
     assert o.guard_cells > 0
+    assert int(res["gpu_guard"].sum()) == st[0]                      # the map and the counter agree
     near = int((np.abs(o.margin) < pu.NEAR_GUARD).sum())
-    assert abs(st[0] - o.guard_cells) <= near, (st, o.guard_cells, near)
+    assert int((res["gpu_guard"] != o.guard).sum()) <= near, (st, o.guard_cells, near)   # only marginal cells flip
 
 
-def test_cfg1_sod_tube_steps_fp32_and_fp64():
-    w = wl.config_1_sod_tube(nx=256, steps=50)
+def test_cfg1_sod_tube_scaled_down_10_steps_fp32_and_fp64():
+    """Fast, scaled-down configs[1] (256 cells = 16 groups, TEN steps, host-driven). The configuration as stated
+    (1024 cells, 64 groups, 200 steps) is tests/test_gpu_configs_full.py::test_cfg1_*."""
+    w = wl.config_1_sod_tube(nx=256, steps=10)
     for dtype, tol in ((np.float32, TOL32_10), (np.float64, 1e-9)):
         dx = pu.f32(w.dx) if dtype == np.float32 else w.dx
         dts = []
@@ -127,7 +134,7 @@ def test_cfg1_sod_tube_steps_fp32_and_fp64():
             dts.append(dt)
             return pu.run_gpu(grp, dt, dx, G, 0, want_bflux=False)[0]
 
-        Ug, t, _ = wl.advance(w.U.astype(dtype), w.dx, w.bc, 0, w.cfl, 10, gpu_step, dtype=dtype)
+        Ug, t, _ = wl.advance(w.U.astype(dtype), w.dx, w.bc, 0, w.cfl, w.steps, gpu_step, dtype=dtype)
         Uo = w.U.astype(np.float64)
         for dt in dts:
             r = O.step_groups(wl.cut_groups(Uo, w.bc), 16, 2, dt, dx, G, 0, want_bflux=False, want_guard=False)
@@ -206,8 +213,8 @@ def test_mirror_symmetry_gpu():
         assert metrics.max_rel_err(back, a, G) <= 2e-6
 
 
-def test_cfg4_sedov_blast_fp64_and_fp32():
-    """configs[4] scaled to 64^3 (64 groups), 100 steps at C = 0.4 on the GPU: positivity of rho and P at every
+def test_cfg4_sedov_blast_scaled_down_fp64_and_fp32():
+    """Fast version: configs[4] scaled to 64^3 (64 groups; the stated 256^3 is tests/test_gpu_configs_full.py), 100 steps at C = 0.4 on the GPU: positivity of rho and P at every
     step, the Sedov-Taylor radius and exponent of pin P15, fp64 parity with the oracle run on the same dt sequence."""
     golden = {}
     import os
@@ -260,7 +267,7 @@ def test_cfg4_sedov_blast_fp64_and_fp32():
 
 def test_headline_full_size_in_the_bench_launch_configuration():
     """BASELINE.json:configs[3] at FULL size (32768 groups, the batch and launch geometry bench.py times, default
-    kernel path): sampled groups — seeded random ones plus those holding the extreme densities — against the
+    kernel path): 2048 sampled groups — seeded random ones plus those holding the extreme densities — against the
     oracle element by element, and properties that hold at any size: finite output everywhere, the per-group flux
     balance (pin P11) on every group, guard count equal to the oracle's on the sample up to marginal cells."""
     w = wl.config_3_cosmo(512, seed=3)
@@ -272,10 +279,16 @@ def test_headline_full_size_in_the_bench_launch_configuration():
     x = torch.from_numpy(grp).to(dev)
     out = torch.full((n, 5, 16, 16, 16), float("nan"), dtype=torch.float32, device=dev)
     bf = torch.full((n, 6, 5, 16, 16), float("nan"), dtype=torch.float32, device=dev)
+    gm = torch.zeros((n, 18, 18, 18), dtype=torch.uint8, device=dev)
     gh.gamer_hydro_status()
-    gh.gamer_hydro_step(x, out, bf, n, 16, 2, dt, dx, G, w.limiter)
-    torch.cuda.synchronize()
+    gh.gamer_hydro_set_guard_map(gm)
+    try:
+        gh.gamer_hydro_step(x, out, bf, n, 16, 2, dt, dx, G, w.limiter)
+        torch.cuda.synchronize()
+    finally:
+        gh.gamer_hydro_set_guard_map(None)
     guard_gpu, nonpos = gh.gamer_hydro_status()
+    assert int(gm.sum()) == guard_gpu
     assert bool(torch.isfinite(out).all()) and bool(torch.isfinite(bf).all())
     # P11 on every group, on the device in fp64: sum(U_out - U_in) = -lambda * (F_hi - F_lo summed over the faces)
     lam = dt / dx
@@ -290,9 +303,10 @@ def test_headline_full_size_in_the_bench_launch_configuration():
     rho_max = grp[:, 0].reshape(n, -1).max(axis=1)
     rho_min = grp[:, 0].reshape(n, -1).min(axis=1)
     rng = np.random.default_rng(2026)
-    idx = np.unique(np.concatenate([rng.choice(n, 96, replace=False), [rho_max.argmax(), rho_min.argmin(), 0, n - 1]]))
-    res = pu.compare(grp[idx], dt, dx, G, w.limiter, out[idx].cpu().numpy(), bf[idx].cpu().numpy())
-    assert res["excluded_fraction"] <= 1e-3, res["excluded_fraction"]
+    idx = np.unique(np.concatenate([rng.choice(n, 2044, replace=False), [rho_max.argmax(), rho_min.argmin(), 0, n - 1]]))
+    res = pu.compare(grp[idx], dt, dx, G, w.limiter, out[idx].cpu().numpy(), bf[idx].cpu().numpy(),
+                     gpu_guard=gm[idx].cpu().numpy())
+    assert res["excluded_fraction"] <= 1e-5, res["excluded_fraction"]
     assert res["err"] <= TOL32_1, res["err"]
     assert res["err_bflux"] <= 10 * TOL32_1, res["err_bflux"]
     assert nonpos == 0
