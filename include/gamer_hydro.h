@@ -10,6 +10,15 @@
  * The numerical details the paper leaves open are fixed in DESIGN.md §3 (readings R1–R21).
  *
  * All functions: extern "C", never throw, never exit; return 0 on success or a GAMER_HYDRO_* code.
+ * Concurrency: the library serves ONE device per process (the first one it is used on; a second device returns
+ * GAMER_HYDRO_INVALID_ARG: run one process per GPU). gamer_hydro_step / _f64, gamer_hydro_max_speed,
+ * gamer_hydro_fill_ghosts, gamer_hydro_step_grid and gamer_hydro_advance may be called concurrently from several
+ * host threads on different streams: every call that reduces on the device takes its own reduction slot (64 in
+ * flight), and calls that need the library's one scratch buffer (the shape-generic kernels) are chained by an event,
+ * i.e. they run one after the other. Process-global and NOT thread-safe: gamer_hydro_set_path,
+ * gamer_hydro_set_guard_map, gamer_hydro_status (test / diagnostic plumbing), gamer_hydro_step_host (it owns the
+ * library's three internal streams) and gamer_hydro_advance on the DUO path (it ping-pongs with one library-owned
+ * array).
  * Pointers are DEVICE pointers unless the name says host. Nothing here takes or returns a torch type.
  *
  * Layouts (x fastest, then y, then z; `real` = float or double):
@@ -119,11 +128,14 @@ int gamer_hydro_step_grid(const float* U_with_ghosts, float* U_out, float* bound
 
 /* n_steps time steps of the fp32 path on one uniform grid without leaving the device: per step
  * dt = float(cfl * dx / max signal speed) (fp64 on the host from the device-side maximum, R15/R11), then
- * gamer_hydro_step, then gamer_hydro_fill_ghosts. U (ghost shells filled on entry) holds the final state with
+ * gamer_hydro_step, then the ghost refill of gamer_hydro_fill_ghosts (whose kernel also accumulates the next maximum). U (ghost shells filled on entry) holds the final state with
  * refilled ghost shells on return, U_out the interiors of the last step, boundary_fluxes (may be NULL) those of
  * the last step; h_dts (HOST, n_steps floats, may be NULL) receives the time steps taken. One 4-byte
- * device-to-host read and one stream synchronisation per step. On a fully periodic grid of 16^3 groups the loop uses
- * gamer_hydro_step_grid, ping-ponging between U and a second ghosted array the library allocates (and keeps). */
+ * device-to-host read and one stream synchronisation per step. With GAMER_HYDRO_PATH_FUSED_DUO selected, a fully
+ * periodic grid of 16^3 groups uses gamer_hydro_step_grid instead of step + refill, ping-ponging between U and a
+ * second ghosted array the library allocates (and keeps). A state without a finite positive signal speed (a NaN or
+ * non-positive cell makes the device maximum NaN) ends the loop with GAMER_HYDRO_INVALID_ARG; on every return,
+ * error or not, U holds the state after the steps completed so far. */
 int gamer_hydro_advance(float* U_with_ghosts, float* U_out, float* boundary_fluxes, int gx, int gy, int gz, int N,
                         int ghost, int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dx, float gamma,
                         int limiter, float* h_dts, cudaStream_t stream);

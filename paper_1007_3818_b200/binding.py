@@ -92,6 +92,12 @@ def _step(fn, dtype, U_in, U_out, boundary_fluxes, N, ghost, dt, dx, gamma, limi
             raise GamerHydroError("tensors must be contiguous CUDA tensors of dtype %s" % dtype)
     if U_out is None:
         U_out = torch.empty((G, 5, N, N, N), dtype=dtype, device=U_in.device)
+    if tuple(U_out.shape) != (G, 5, N, N, N):
+        raise GamerHydroError("U_out must be [%d][5][%d][%d][%d], got %s" % (G, N, N, N, tuple(U_out.shape)))
+    if boundary_fluxes is not None and tuple(boundary_fluxes.shape) != (G, 6, 5, N, N):
+        raise GamerHydroError("boundary_fluxes must be [%d][6][5][%d][%d], got %s" % (G, N, N, tuple(boundary_fluxes.shape)))
+    if any(x is not None and x.device != U_in.device for x in (U_out, boundary_fluxes)):
+        raise GamerHydroError("all tensors must live on the same CUDA device")
     bf = boundary_fluxes.data_ptr() if boundary_fluxes is not None else None
     _check(fn(U_in.data_ptr(), U_out.data_ptr(), bf, G, N, ghost, dt, dx, gamma, int(limiter), _stream_ptr(stream)))
     return U_out

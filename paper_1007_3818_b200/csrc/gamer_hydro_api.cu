@@ -29,9 +29,11 @@ struct State {
   int device = -1;
   int sm_count = 0;
   int smem_per_sm = 0;
-  unsigned long long* status = nullptr;  // [0] guard cells, [1] non-positive outputs
+  unsigned long long* status = nullptr;  // [0] guard cells, [1] non-positive outputs, [2 ..] per-call reduction slots
   void* scratch = nullptr;               // generic path: FS + FL for `scratch_groups` groups
   size_t scratch_bytes = 0;
+  cudaEvent_t scratch_free = nullptr;    // recorded after the last reader of the scratch: the next user waits on it
+  bool scratch_used = false;
   // host-buffer path
   cudaStream_t hstream[3] = {nullptr, nullptr, nullptr};
   void* hbuf_in[3] = {nullptr, nullptr, nullptr};
@@ -49,6 +51,13 @@ struct State {
 State g_state;
 std::mutex g_mutex;
 std::atomic<unsigned long long> g_launches{0};
+std::atomic<unsigned int> g_slot{0};
+
+constexpr int kReduceSlots = 64;    // signal-speed maxima of concurrent max_speed / step_grid / advance calls
+
+// every call that reduces a signal-speed maximum on the device takes its own 8-byte slot (round robin), so calls on
+// different streams do not share one
+unsigned long long* next_reduce_slot() { return g_state.status + 2 + (g_slot.fetch_add(1) % kReduceSlots); }
 
 constexpr int kGenericChunk = 512;  // groups per generic-path launch (bounds the scratch buffer)
 
@@ -82,8 +91,9 @@ int init_locked(int device) {
   g_state.sm_count = prop.multiProcessorCount;
   g_state.smem_per_sm = (int)prop.sharedMemPerMultiprocessor;
   // [0] guard cells, [1] non-positive outputs, [2] bit pattern of the running signal-speed maximum
-  CK(cudaMalloc(&g_state.status, 4 * sizeof(unsigned long long)));
-  CK(cudaMemset(g_state.status, 0, 4 * sizeof(unsigned long long)));
+  CK(cudaMalloc(&g_state.status, (2 + kReduceSlots) * sizeof(unsigned long long)));
+  CK(cudaMemset(g_state.status, 0, (2 + kReduceSlots) * sizeof(unsigned long long)));
+  CK(cudaEventCreateWithFlags(&g_state.scratch_free, cudaEventDisableTiming));
   int rc;
   if ((rc = set_fused_attr<float, 0, true>())) return rc;
   if ((rc = set_fused_attr<float, 1, true>())) return rc;
@@ -256,6 +266,10 @@ int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int g
   R* FS = reinterpret_cast<R*>(g_state.scratch);
   R* FL = FS + (size_t)chunk * sh.fs_stride;
   const long long ne = (long long)sh.E * sh.E * sh.E, nf = 3LL * (N + 1) * N * N, nc = (long long)N * N * N;
+  // ONE scratch buffer serves every stream: calls on different streams are chained by an event (the predictor of the
+  // next call waits for the update kernel of the previous one), under the lock so that the chain is a total order
+  std::lock_guard<std::mutex> lk(g_mutex);
+  if (g_state.scratch_used) CK(cudaStreamWaitEvent(stream, g_state.scratch_free, 0));
   for (int g0 = 0; g0 < n_groups; g0 += chunk) {
     const int ng = (n_groups - g0) < chunk ? (n_groups - g0) : chunk;
     const R* in = U_in + (size_t)g0 * sh.in_stride;
@@ -270,6 +284,8 @@ int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int g
     g_launches.fetch_add(3);
   }
   CK(cudaGetLastError());
+  CK(cudaEventRecord(g_state.scratch_free, stream));
+  g_state.scratch_used = true;
   return 0;
 }
 
@@ -317,7 +333,7 @@ int max_speed_impl(const R* U, int n_groups, int N, int ghost, double gamma, dou
   if (n_groups == 0) return 0;
   int rc = ensure_init();
   if (rc) return rc;
-  Bits* slot = reinterpret_cast<Bits*>(g_state.status + 2);
+  Bits* slot = reinterpret_cast<Bits*>(next_reduce_slot());
   CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
   const long long n_cells = (long long)n_groups * N * N * N;
   const int threads = 256;
@@ -338,7 +354,7 @@ int max_speed_impl(const R* U, int n_groups, int N, int ghost, double gamma, dou
 // want_max: also accumulate the signal-speed maximum of the refilled state into the status slot (zeroed first)
 template <class R, class Bits>
 int fill_ghosts_impl(const R* U_out, R* U_in, int gx, int gy, int gz, int N, int ghost, int bcx, int bcy, int bcz,
-                     cudaStream_t stream, bool want_max = false, double gamma = 5.0 / 3.0) {
+                     cudaStream_t stream, unsigned long long* max_slot = nullptr, double gamma = 5.0 / 3.0) {
   if (!U_out || !U_in || gx < 1 || gy < 1 || gz < 1 || N < 1 || ghost < 0 || (bcx | bcy | bcz) < 0 || bcx > 1 ||
       bcy > 1 || bcz > 1)
     return GAMER_HYDRO_INVALID_ARG;
@@ -347,8 +363,8 @@ int fill_ghosts_impl(const R* U_out, R* U_in, int gx, int gy, int gz, int N, int
   int rc = ensure_init();
   if (rc) return rc;
   Bits* slot = nullptr;
-  if (want_max) {
-    slot = reinterpret_cast<Bits*>(g_state.status + 2);
+  if (max_slot) {
+    slot = reinterpret_cast<Bits*>(max_slot);
     CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
   }
   const int grid = gx * gy * gz;   // one CTA per group
@@ -435,8 +451,9 @@ int gamer_hydro_fill_ghosts(const void* U_out, void* U_in_with_ghosts, int bytes
   return GAMER_HYDRO_INVALID_ARG;
 }
 
-int gamer_hydro_step_grid(const float* U, float* U_out, float* bflux, float* U_next, int gx, int gy, int gz, int N,
-                          int ghost, float dt, float dx, float gamma, int limiter, cudaStream_t stream) {
+static int step_grid_impl(const float* U, float* U_out, float* bflux, float* U_next, int gx, int gy, int gz, int N,
+                          int ghost, float dt, float dx, float gamma, int limiter, cudaStream_t stream,
+                          unsigned long long* max_slot) {
   if (gx < 1 || gy < 1 || gz < 1 || (long long)gx * gy * gz > 0x7fffffffLL || !U_next || U_next == U)
     return GAMER_HYDRO_INVALID_ARG;
   const int ng = gx * gy * gz;
@@ -444,10 +461,15 @@ int gamer_hydro_step_grid(const float* U, float* U_out, float* bflux, float* U_n
   if (rc) return rc;
   if (N != gh::FN || ghost != 2) return GAMER_HYDRO_UNSUPPORTED;   // the fused-halo kernel is the N = 16, ghost = 2 one
   if ((rc = ensure_init())) return rc;
-  unsigned int* slot = reinterpret_cast<unsigned int*>(g_state.status + 2);
+  unsigned int* slot = reinterpret_cast<unsigned int*>(max_slot ? max_slot : next_reduce_slot());
   CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
   const gh::HaloGrid hg = {U_next, slot, gx, gy, gz};
   return launch_duo(U, U_out, bflux, ng, N, ghost, dt, dx, gamma, limiter, stream, &hg);
+}
+
+int gamer_hydro_step_grid(const float* U, float* U_out, float* bflux, float* U_next, int gx, int gy, int gz, int N,
+                          int ghost, float dt, float dx, float gamma, int limiter, cudaStream_t stream) {
+  return step_grid_impl(U, U_out, bflux, U_next, gx, gy, gz, N, ghost, dt, dx, gamma, limiter, stream, nullptr);
 }
 
 int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, int gz, int N, int ghost, int bc_x,
@@ -462,53 +484,62 @@ int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, in
   double vmax = 0.0;
   int rc = gamer_hydro_max_speed(U, 4, (int)ng, N, ghost, (double)gamma, &vmax, stream);   // state on entry
   if (rc) return rc;
+  unsigned long long* const slot = next_reduce_slot();   // this call's own reduction slot (calls on other streams take others)
   // Default: step + ghost refill (the refill pass also accumulates the next signal-speed maximum). With the DUO path
   // selected, a fully periodic grid of 16^3 groups uses the fused-halo variant of that kernel instead: the step
   // kernel itself writes the next step's ghosted array and signal-speed maximum (ping-pong between U and a
-  // library-owned second array).
+  // library-owned second array; that array is shared, so this variant is not re-entrant).
   const bool fused_halo = bc_x == 0 && bc_y == 0 && bc_z == 0 && N == gh::FN && ghost == 2 &&
                           g_state.path == GAMER_HYDRO_PATH_FUSED_DUO;
+  const size_t grid_bytes = (size_t)ng * 5 * 20 * 20 * 20 * sizeof(float);
   float* cur = U;
   float* nxt = nullptr;
   if (fused_halo) {
-    const size_t bytes = (size_t)ng * 5 * 20 * 20 * 20 * sizeof(float);
     std::lock_guard<std::mutex> lk(g_mutex);
-    if (g_state.grid_buf_bytes < bytes) {
+    if (g_state.grid_buf_bytes < grid_bytes) {
       CK(cudaDeviceSynchronize());
       if (g_state.grid_buf) cudaFree(g_state.grid_buf);
       g_state.grid_buf = nullptr;
       g_state.grid_buf_bytes = 0;
-      CK(cudaMalloc(&g_state.grid_buf, bytes));
-      g_state.grid_buf_bytes = bytes;
+      CK(cudaMalloc(&g_state.grid_buf, grid_bytes));
+      g_state.grid_buf_bytes = grid_bytes;
     }
     nxt = (float*)g_state.grid_buf;
   }
+  // on ANY exit the caller's U holds the state after the steps completed so far (never a stale ping-pong buffer)
+  auto finish = [&](int code) -> int {
+    if (cur != U) {
+      if (cudaMemcpyAsync(U, cur, grid_bytes, cudaMemcpyDeviceToDevice, stream) != cudaSuccess ||
+          cudaStreamSynchronize(stream) != cudaSuccess)
+        return code ? code : cuda_fail(cudaGetLastError(), "copy of the final state back to U");
+    }
+    return code;
+  };
   for (int s = 0; s < n_steps; ++s) {
-    if (!(vmax > 0.0) || vmax > 3.0e38) return GAMER_HYDRO_INVALID_ARG;   // no finite positive signal speed: invalid state
+    // no finite positive signal speed (a NaN state reduces to NaN: the device maximum propagates it): invalid state
+    if (!(vmax > 0.0) || vmax > 3.0e38) return finish(GAMER_HYDRO_INVALID_ARG);
     const float dt = (float)((double)cfl * (double)dx / vmax);            // R15, fp64 on the host, rounded once (R11)
     if (h_dts) h_dts[s] = dt;
     if (fused_halo) {
-      if ((rc = gamer_hydro_step_grid(cur, U_out, bflux, nxt, gx, gy, gz, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
+      if ((rc = step_grid_impl(cur, U_out, bflux, nxt, gx, gy, gz, N, ghost, dt, dx, gamma, limiter, stream, slot)))
+        return finish(rc);
       float* tmp = cur; cur = nxt; nxt = tmp;
     } else {
       if ((rc = gamer_hydro_step(U, U_out, bflux, (int)ng, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
       // ghost refill fused with the signal-speed maximum of the new state (next step's dt)
-      if ((rc = fill_ghosts_impl<float, unsigned int>(U_out, U, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream, true,
+      if ((rc = fill_ghosts_impl<float, unsigned int>(U_out, U, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream, slot,
                                                       (double)gamma)))
         return rc;
     }
     unsigned int bits = 0;
-    CK(cudaMemcpyAsync(&bits, g_state.status + 2, sizeof(bits), cudaMemcpyDeviceToHost, stream));
-    CK(cudaStreamSynchronize(stream));
+    if (cudaMemcpyAsync(&bits, slot, sizeof(bits), cudaMemcpyDeviceToHost, stream) != cudaSuccess ||
+        cudaStreamSynchronize(stream) != cudaSuccess)
+      return finish(cuda_fail(cudaGetLastError(), "read of the signal-speed maximum"));
     float v;
     memcpy(&v, &bits, sizeof(v));
     vmax = (double)v;
   }
-  if (cur != U) {  // odd number of fused steps: the final state sits in the library's array
-    CK(cudaMemcpyAsync(U, cur, (size_t)ng * 5 * 20 * 20 * 20 * sizeof(float), cudaMemcpyDeviceToDevice, stream));
-    CK(cudaStreamSynchronize(stream));
-  }
-  return 0;
+  return finish(0);
 }
 
 int gamer_hydro_step_host(const float* h_in, float* h_out, float* h_bf, int n_groups, int N, int ghost, float dt,

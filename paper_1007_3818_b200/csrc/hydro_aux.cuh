@@ -9,7 +9,8 @@ namespace gh {
 
 // max over the interior cells of all groups of |vx| + |vy| + |vz| + 3 c_s (R15). U: [G][5][S][S][S] with
 // S = N + 2 ghost (ghost = 0 for U_out). The result is accumulated with an integer atomicMax on the bit pattern
-// (non-negative IEEE values order like unsigned integers), so *out must be zeroed before the launch.
+// (non-negative IEEE values order like unsigned integers; a NaN orders above them all, so a state holding NaN gives
+// a NaN maximum and the caller's dt check trips), so *out must be zeroed before the launch.
 template <class R, class Bits>
 __global__ void max_speed_kernel(const R* __restrict__ U, long long n_cells, int N, int ghost, R gamma, Bits* out) {
   const int S = N + 2 * ghost;
@@ -25,11 +26,11 @@ __global__ void max_speed_kernel(const R* __restrict__ U, long long n_cells, int
     R P = (gamma - R(1)) * (E - R(0.5) * (mx * mx + my * my + mz * mz) * ir);
     P = P > R(0) ? P : R(0);
     const R v = (fabs(mx) + fabs(my) + fabs(mz)) * ir + R(3) * sqrt(gamma * P * ir);
-    m = v > m ? v : m;   // NaN never wins
+    m = (v > m || v != v) ? v : m;   // a NaN cell makes the maximum NaN (its bit pattern also wins the atomicMax)
   }
   for (int o = 16; o > 0; o >>= 1) {
     const R other = __shfl_xor_sync(0xffffffffu, m, o);
-    m = other > m ? other : m;
+    m = (other > m || other != other) ? other : m;
   }
   if ((threadIdx.x & 31) == 0) {
     Bits b;
@@ -105,14 +106,14 @@ __global__ void fill_ghosts_kernel(const R* __restrict__ U_out, R* __restrict__ 
         R P = (gamma - R(1)) * (v[e][4] - R(0.5) * (v[e][1] * v[e][1] + v[e][2] * v[e][2] + v[e][3] * v[e][3]) * ir);
         P = P > R(0) ? P : R(0);
         const R sp = (fabs(v[e][1]) + fabs(v[e][2]) + fabs(v[e][3])) * ir + R(3) * sqrt(gamma * P * ir);
-        m = sp > m ? sp : m;
+        m = (sp > m || sp != sp) ? sp : m;
       }
     }
   }
   if (vmax) {
     for (int o = 16; o > 0; o >>= 1) {
       const R other = __shfl_xor_sync(0xffffffffu, m, o);
-      m = other > m ? other : m;
+      m = (other > m || other != other) ? other : m;
     }
     if ((threadIdx.x & 31) == 0) {
       Bits b;

@@ -426,7 +426,7 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
           const float ir = rcp1(out[0]);
           const float P = fmaxf(lo(c.g1) * fmaf(-0.5f * m2, ir, out[4]), 0.0f);
           const float sp = (fabsf(out[1]) + fabsf(out[2]) + fabsf(out[3])) * ir + 3.0f * sqrt1((lo(c.g1) + 1.0f) * P * ir);
-          vmax_thread = sp > vmax_thread ? sp : vmax_thread;
+          vmax_thread = (sp > vmax_thread || sp != sp) ? sp : vmax_thread;
           // the cell in the next step's ghosted array: own interior position, and the ghost shells of the neighbours
           // it is within two cells of (per axis: none, or the one at -1 / +1)
           const int kk = k - 1;
@@ -502,7 +502,7 @@ __device__ __forceinline__ void duo_half(const CUtensorMap& in_map, float* __res
   if (HALO) {
     for (int o = 16; o > 0; o >>= 1) {
       const float other = __shfl_xor_sync(0xffffffffu, vmax_thread, o);
-      vmax_thread = other > vmax_thread ? other : vmax_thread;
+      vmax_thread = (other > vmax_thread || other != other) ? other : vmax_thread;
     }
     if ((t & 31) == 0) atomicMax(hg.vmax, __float_as_uint(vmax_thread));
   }

@@ -222,3 +222,46 @@ def test_fused_halo_step_on_the_guard_heavy_cosmo_field():
     vnew = gh.gamer_hydro_max_speed(torch.from_numpy(res[1][0]).to(DEV), ghost=0)
     # (advance's first step used its own dt, so only check the relation dt = cfl dx / vmax on the second step loosely)
     assert dts[1] > 0 and np.isfinite(vnew)
+
+
+def test_two_advance_loops_on_two_streams_give_the_single_stream_bits():
+    """SURVEY.md 8(b) 're-entrant across streams': two gamer_hydro_advance loops (different grids, different streams,
+    two host threads — ctypes releases the GIL inside the call) running concurrently give the bits of the same loops run
+    one after the other: every call reduces its signal-speed maximum in its own slot."""
+    import threading
+    ws = [wl.config_2_turbulence(64, seed=21, steps=8), wl.config_3_cosmo(64, seed=22)]
+    steps = 8
+
+    def run(w, stream, out):
+        with torch.cuda.stream(stream):
+            d_U = torch.from_numpy(w.groups()).to(DEV)
+            d_out = torch.empty((d_U.shape[0], 5, 16, 16, 16), dtype=torch.float32, device=DEV)
+            dts = gh.gamer_hydro_advance(d_U, d_out, None, _grid(w.shape), steps, 0.4, pu.f32(w.dx),
+                                         bc=[BC[b] for b in w.bc], limiter=w.limiter, stream=stream)
+            stream.synchronize()
+            out.append((dts, d_out.cpu().numpy(), d_U.cpu().numpy()))
+
+    serial = [[], []]
+    for k, w in enumerate(ws):
+        run(w, torch.cuda.Stream(), serial[k])
+    for rep in range(3):
+        conc = [[], []]
+        th = [threading.Thread(target=run, args=(w, torch.cuda.Stream(), conc[k])) for k, w in enumerate(ws)]
+        for t in th:
+            t.start()
+        for t in th:
+            t.join()
+        for k in range(2):
+            assert conc[k][0][0] == serial[k][0][0]                              # same dt sequence
+            assert np.array_equal(conc[k][0][1], serial[k][0][1]) and np.array_equal(conc[k][0][2], serial[k][0][2])
+
+
+def test_advance_reports_a_nan_state_and_leaves_the_completed_steps_in_U():
+    w = wl.config_2_turbulence(32, seed=23)
+    d_U = torch.from_numpy(w.groups()).to(DEV)
+    n = d_U.shape[0]
+    d_out = torch.empty((n, 5, 16, 16, 16), dtype=torch.float32, device=DEV)
+    d_U[3, 4, 9, 9, 9] = float("nan")                      # one interior cell: the device maximum must become NaN
+    with pytest.raises(gh.GamerHydroError):
+        gh.gamer_hydro_advance(d_U, d_out, None, _grid(w.shape), 3, 0.4, pu.f32(w.dx), limiter=w.limiter)
+    assert np.isnan(gh.gamer_hydro_max_speed(d_U))

@@ -346,3 +346,51 @@ def test_repeated_launches_are_bit_identical(path):
         assert torch.equal(out.view(torch.int32), ref_out[n - m:].view(torch.int32))
     finally:
         gh.gamer_hydro_set_path(gh.PATH_AUTO)
+
+
+def test_host_buffer_entry_point_generic_shape_ragged_chunks_pageable_and_null_fluxes():
+    """gamer_hydro_step_host on a shape served by the generic kernels (N = 8, ghost = 3: ONE scratch buffer shared by
+    the three internal streams, chained by an event), with n_groups far above and not a multiple of the chunk, pageable
+    host memory and boundary_fluxes == NULL: same bits as the device path, and as the oracle within tolerance."""
+    g8 = wl.random_groups(203, seed=109, N=8, ghost=3)
+    dt, dx = pu.f32(2e-3), pu.f32(1 / 8)
+    dev_out, dev_bf, _ = pu.run_gpu(g8, dt, dx, G, 1, N=8, ghost=3)
+    for pinned in (True, False):
+        h_in = torch.from_numpy(g8.copy())
+        h_out = torch.full((203, 5, 8, 8, 8), float("nan"), dtype=torch.float32)
+        h_bf = torch.full((203, 6, 5, 8, 8), float("nan"), dtype=torch.float32)
+        if pinned:
+            h_in, h_out, h_bf = h_in.pin_memory(), h_out.pin_memory(), h_bf.pin_memory()
+        for rep in range(3):        # repeated: a race on the shared scratch would show as a changed bit sooner or later
+            gh.gamer_hydro_step_host(h_in, h_out, h_bf, 203, 8, 3, dt, dx, G, 1, chunk_groups=16)
+            assert np.array_equal(h_out.numpy(), dev_out) and np.array_equal(h_bf.numpy(), dev_bf)
+    h_out2 = torch.full((203, 5, 8, 8, 8), float("nan"), dtype=torch.float32).pin_memory()
+    gh.gamer_hydro_step_host(torch.from_numpy(g8).pin_memory(), h_out2, None, 203, 8, 3, dt, dx, G, 1, chunk_groups=7)
+    assert np.array_equal(h_out2.numpy(), dev_out)
+    r = O.step_groups(g8, 8, 3, dt, dx, G, 1)
+    assert metrics.max_rel_err(dev_out, r.U_out, G) <= TOL32_1
+    # the fused path with a ragged last chunk too
+    g = wl.random_groups(37, seed=110)
+    a = pu.run_gpu(g, pu.f32(2e-3), pu.f32(1 / 16), G, 0)
+    h_out3 = torch.empty((37, 5, 16, 16, 16), dtype=torch.float32)
+    gh.gamer_hydro_step_host(torch.from_numpy(g), h_out3, None, 37, 16, 2, pu.f32(2e-3), pu.f32(1 / 16), G, 0, chunk_groups=10)
+    assert np.array_equal(h_out3.numpy(), a[0])
+
+
+def test_two_streams_on_the_generic_path_do_not_race_on_the_scratch():
+    """Two user streams calling gamer_hydro_step on a generic shape: the calls share the library's scratch buffer and
+    must be serialised by it (advisor finding, round 1)."""
+    dev = torch.device("cuda", 0)
+    ga, gb = wl.random_groups(300, seed=111, N=8, ghost=3), wl.random_groups(300, seed=112, N=8, ghost=3)
+    dt, dx = pu.f32(2e-3), pu.f32(1 / 8)
+    ref = [pu.run_gpu(g, dt, dx, G, 0, N=8, ghost=3)[0] for g in (ga, gb)]
+    xa, xb = torch.from_numpy(ga).to(dev), torch.from_numpy(gb).to(dev)
+    for rep in range(5):
+        oa = torch.full((300, 5, 8, 8, 8), float("nan"), device=dev)
+        ob = torch.full((300, 5, 8, 8, 8), float("nan"), device=dev)
+        sa, sb = torch.cuda.Stream(), torch.cuda.Stream()
+        torch.cuda.synchronize()
+        gh.gamer_hydro_step(xa, oa, None, 300, 8, 3, dt, dx, G, 0, stream=sa)
+        gh.gamer_hydro_step(xb, ob, None, 300, 8, 3, dt, dx, G, 0, stream=sb)
+        torch.cuda.synchronize()
+        assert np.array_equal(oa.cpu().numpy(), ref[0]) and np.array_equal(ob.cpu().numpy(), ref[1])
