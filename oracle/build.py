@@ -29,5 +29,23 @@ def build(force: bool = False) -> str:
     return LIB
 
 
+RTVD_SOURCES = ["rtvd_oracle_capi.cpp", "rtvd_oracle.hpp"]
+RTVD_LIB = os.path.join(HERE, "librtvd_oracle.so")
+
+
+def build_rtvd(force: bool = False) -> str:
+    """The relaxing-TVD oracle, same flags, its own library."""
+    stale = not os.path.exists(RTVD_LIB) or any(os.path.getmtime(os.path.join(HERE, s)) > os.path.getmtime(RTVD_LIB)
+                                                for s in RTVD_SOURCES)
+    if force or stale:
+        tmp = RTVD_LIB + ".tmp.%d" % os.getpid()
+        cmd = ["g++", "-std=c++17", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC", "-Wall",
+               "-o", tmp, os.path.join(HERE, "rtvd_oracle_capi.cpp")]
+        subprocess.run(cmd, check=True, cwd=HERE)
+        os.replace(tmp, RTVD_LIB)
+    return RTVD_LIB
+
+
 if __name__ == "__main__":
+    print(build_rtvd(force=True))
     print(build(force=True))
