@@ -140,6 +140,19 @@ int gamer_hydro_advance(float* U_with_ghosts, float* U_out, float* boundary_flux
                         int ghost, int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dx, float gamma,
                         int limiter, float* h_dts, cudaStream_t stream);
 
+/* ---- second workload: the relaxing-TVD solver. PAPER.md:13 (§2): "the second-order relaxing
+ * total variation diminishing (TVD) method (Trac & Pen 2003)", dimensionally split; it needs "seven points"
+ * per direction, i.e. THREE ghost cells. One call = one time step of every group: three 1-D sweeps with the full dt, in
+ * the order x, y, z (sweep = 0) or z, y, x (sweep = 1; callers alternate). Each sweep: half step with the first-order
+ * upwind fluxes of the relaxed system (freezing speed |v| + c_s per cell), full step with van-Leer-limited second-order
+ * fluxes on the half-step state (readings RT1–RT8). fp32.
+ *   U_in_with_ghosts  float[n_groups][5][S][S][S], S = N + 2*ghost, DEVICE, 16-byte aligned, read-only
+ *   U_out             float[n_groups][5][N][N][N], DEVICE, must not alias U_in
+ * N = 16 and ghost = 3 only (GAMER_HYDRO_UNSUPPORTED otherwise); no boundary fluxes (RT7). Enqueues on `stream` and
+ * returns; re-entrant across streams; deterministic. Errors as gamer_hydro_step. */
+int gamer_rtvd_step(const float* U_in_with_ghosts, float* U_out, int n_groups, int N, int ghost, float dt, float dx,
+                    float gamma, int sweep, cudaStream_t stream);
+
 /* Diagnostics accumulated since the last call (and reset by it): number of cells whose predicted face
  * states failed the positivity guard and fell back to first order (R7), and number of updated
  * cells with rho <= 0 or P <= 0 (R10: counted, never floored). Synchronises the device. Either pointer may

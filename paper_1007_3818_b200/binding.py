@@ -20,7 +20,7 @@ PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_DUO = 0, 1, 2
 EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
            "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance",
-           "gamer_hydro_step_grid", "gamer_hydro_set_guard_map"]
+           "gamer_hydro_step_grid", "gamer_hydro_set_guard_map", "gamer_rtvd_step"]
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
@@ -49,6 +49,7 @@ def lib():
         L.gamer_hydro_step_grid.argtypes = [vp, vp, vp, vp, i, i, i, i, i, f, f, f, i, vp]
         L.gamer_hydro_advance.argtypes = [vp, vp, vp, i, i, i, i, i, i, i, i, i, f, f, f, i, vp, vp]
         L.gamer_hydro_set_guard_map.argtypes = [vp]
+        L.gamer_rtvd_step.argtypes = [vp, vp, i, i, i, f, f, f, i, vp]
         L.gamer_hydro_launch_count.restype = C.c_ulonglong
         L.gamer_hydro_strerror.restype = C.c_char_p
         L.gamer_hydro_strerror.argtypes = [i]
@@ -205,6 +206,23 @@ def gamer_hydro_status():
 
 def gamer_hydro_set_path(path):
     _check(lib().gamer_hydro_set_path(int(path)))
+
+
+def gamer_rtvd_step(U_in_with_ghosts, U_out, n_groups=None, N=16, ghost=3, dt=None, dx=None, gamma=5.0 / 3.0, sweep=0,
+                    stream=None):
+    """One relaxing-TVD step (fp32) on device tensors [G][5][N+2*ghost]^3 -> [G][5][N]^3; returns U_out."""
+    G = _shapes(U_in_with_ghosts, N, ghost)
+    assert n_groups is None or n_groups == G
+    if U_out is None:
+        U_out = torch.empty((G, 5, N, N, N), dtype=torch.float32, device=U_in_with_ghosts.device)
+    for x in (U_in_with_ghosts, U_out):
+        if not (x.is_cuda and x.dtype == torch.float32 and x.is_contiguous()):
+            raise GamerHydroError("tensors must be contiguous CUDA float32 tensors")
+    if tuple(U_out.shape) != (G, 5, N, N, N) or U_out.device != U_in_with_ghosts.device:
+        raise GamerHydroError("U_out must be [%d][5][%d][%d][%d] on the device of U_in" % (G, N, N, N))
+    _check(lib().gamer_rtvd_step(U_in_with_ghosts.data_ptr(), U_out.data_ptr(), G, N, ghost, dt, dx, gamma, int(sweep),
+                                 _stream_ptr(stream)))
+    return U_out
 
 
 def gamer_hydro_set_guard_map(device_map):

@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgamer_hydro.so")
 SOURCES = ["gamer_hydro_api.cu"]
-DEPS = ["gamer_hydro_api.cu", "hydro_fused.cuh", "hydro_f2.cuh", "hydro_duo.cuh", "hydro_zpair.cuh", "hydro_aux.cuh", "hydro_generic.cuh", "hydro_math.cuh",
+DEPS = ["gamer_hydro_api.cu", "hydro_fused.cuh", "hydro_f2.cuh", "hydro_duo.cuh", "hydro_zpair.cuh", "hydro_aux.cuh", "hydro_rtvd.cuh", "hydro_generic.cuh", "hydro_math.cuh",
         os.path.join("..", "..", "include", "gamer_hydro.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-shared",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v", "--expt-relaxed-constexpr"]

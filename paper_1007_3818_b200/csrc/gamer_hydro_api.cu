@@ -17,6 +17,7 @@
 #include "hydro_duo.cuh"
 #include "hydro_zpair.cuh"
 #include "hydro_aux.cuh"
+#include "hydro_rtvd.cuh"
 
 namespace {
 
@@ -105,6 +106,8 @@ int init_locked(int device) {
   CK(cudaFuncSetAttribute(gh::duo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_halo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_halo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
+  CK(cudaFuncSetAttribute(gh::rtvd_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::RtvdSmem::total));
+  CK(cudaFuncSetAttribute(gh::rtvd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::RtvdSmem::total));
   void* fn = nullptr;
   cudaDriverEntryPointQueryResult qres;
   CK(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
@@ -585,6 +588,25 @@ int gamer_hydro_step_host(const float* h_in, float* h_out, float* h_bf, int n_gr
       CK(cudaMemcpyAsync(h_bf + (size_t)g0 * bf_g, d_bf, ng * bf_g * sizeof(float), cudaMemcpyDeviceToHost, st));
   }
   for (int s = 0; s < 3; ++s) CK(cudaStreamSynchronize(g_state.hstream[s]));
+  return 0;
+}
+
+int gamer_rtvd_step(const float* U_in, float* U_out, int n_groups, int N, int ghost, float dt, float dx, float gamma,
+                    int sweep, cudaStream_t stream) {
+  if (n_groups < 0 || N < 1 || ghost < 3 || (sweep != 0 && sweep != 1)) return GAMER_HYDRO_INVALID_ARG;
+  if (!(dt > 0.0f) || !(dx > 0.0f) || !isfinite((double)dt) || !isfinite((double)dx)) return GAMER_HYDRO_INVALID_ARG;
+  if (!(gamma > 1.0f) || !isfinite((double)gamma)) return GAMER_HYDRO_INVALID_ARG;
+  if (n_groups == 0) return 0;
+  if (!U_in || !U_out || ((uintptr_t)U_in & 15) || ((uintptr_t)U_out & 15)) return GAMER_HYDRO_INVALID_ARG;
+  if (N != gh::RN || ghost != gh::RG) return GAMER_HYDRO_UNSUPPORTED;   // the kernel holds one 22^3 x 5 tile per CTA
+  int rc = ensure_init();
+  if (rc) return rc;
+  const gh::RtvdConst c = {dt / dx, 0.5f * (dt / dx), gamma - 1.0f, gamma};
+  const int grid = n_groups < g_state.sm_count ? n_groups : g_state.sm_count;   // persistent: one CTA per SM
+  if (sweep == 0) gh::rtvd_kernel<0><<<grid, gh::RNT, gh::RtvdSmem::total, stream>>>(U_in, U_out, n_groups, c);
+  else gh::rtvd_kernel<1><<<grid, gh::RNT, gh::RtvdSmem::total, stream>>>(U_in, U_out, n_groups, c);
+  g_launches.fetch_add(1);
+  CK(cudaGetLastError());
   return 0;
 }
 

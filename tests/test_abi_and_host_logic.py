@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 def declared_functions():
     src = open(os.path.join(ROOT, "include", "gamer_hydro.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(gamer_hydro_[a-z0-9_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(gamer_(?:hydro|rtvd)_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_header_declares_the_north_star_entry_points():
