@@ -41,6 +41,9 @@ N, GHOST = 16, 2
 FLOPS_PER_CELL = {0: 1033.94, 1: 1095.81}
 FLOPS_PER_CELL_HAND = {0: 925.0, 1: 966.0}
 BYTES_PER_CELL = 66.5625           # (5*20^3 + 5*16^3 + 30*16^2) * 4 B / 16^3
+# relaxing-TVD step: hand count of the oracle text, 1092 lines of 22 cells per group
+RTVD_FLOPS_PER_CELL = 1279.0
+RTVD_BYTES_PER_CELL = (5 * 22 ** 3 + 5 * 16 ** 3) * 4 / 16 ** 3      # 72.0
 SM_COUNT, LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = SM_COUNT * LANES * 2 * SM_MAX_GHZ / 1e3     # 74.45
 
@@ -427,6 +430,36 @@ def main():
                      "dt_first": ms_dts[0], "dt_last": ms_dts[-1]}
         del d_state
 
+    # ---- second workload: the relaxing-TVD step on a 256^3 box of the same recipe with 3 ghost
+    # cells (4096 groups), beside the headline, with its own roofline
+    rtvd = None
+    if not args.no_multistep and world == 1:
+        from harness import workloads as wl
+        w2 = wl.config_3_cosmo(min(args.box, 256), seed=args.seed)
+        g3 = torch.from_numpy(wl.cut_groups(w2.U, w2.bc, ghost=3)).to(dev)
+        n3 = g3.shape[0]
+        o3 = torch.empty((n3, 5, N, N, N), dtype=torch.float32, device=dev)
+        dt3, dx3 = float(np.float32(w2.dt())), float(np.float32(w2.dx))
+        for s in range(3):
+            gh.gamer_rtvd_step(g3, o3, n3, N, 3, dt3, dx3, w2.gamma, s % 2, stream=stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for s in range(10):
+            gh.gamer_rtvd_step(g3, o3, n3, N, 3, dt3, dx3, w2.gamma, s % 2, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms3 = e0.elapsed_time(e1) / 10
+        c3 = n3 * N ** 3
+        rtvd = {"value": c3 / (ms3 * 1e-3), "unit": UNIT, "ms_per_step": ms3, "groups": n3, "ghost": 3,
+                "api": "gamer_rtvd_step (x,y,z / z,y,x sweeps alternating)", "kernel": "gh::rtvd_kernel",
+                "roofline": {"bound": "alu", "flops_per_cell_update": RTVD_FLOPS_PER_CELL,
+                             "achieved": RTVD_FLOPS_PER_CELL * c3 / (ms3 * 1e-3) / 1e12, "peak": ALU_PEAK_TFLOPS,
+                             "unit": "TFLOP/s", "frac": RTVD_FLOPS_PER_CELL * c3 / (ms3 * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,
+                             "hbm_bytes_per_cell_update": RTVD_BYTES_PER_CELL,
+                             "hbm_frac": RTVD_BYTES_PER_CELL * c3 / (ms3 * 1e-3) / 1e9 / hbm_peak}}
+        del g3, o3
+
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
            "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -439,7 +472,7 @@ def main():
                                      ("the one batch split into contiguous ranges" if args.scaling == "strong" and world > 1
                                       else "the full batch on every rank"),
                       "generation_seconds": gen_s, "dt": dt, "dx": dx, "kernel_path": args.path},
-           "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "multistep": multistep,
+           "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "multistep": multistep, "rtvd": rtvd,
            "gpu_launches": int(launches),
            "clocks": clocks, "ms_per_step_min": min(per_step), "ms_per_step_median": float(np.median(per_step)),
            "guard_cells_per_step": guard_cells / args.steps, "nonpositive_out_per_step": nonpos / args.steps,

@@ -31,7 +31,10 @@
 
 namespace mhm_oracle {
 
-enum Limiter { MINMOD = 0, VANLEER = 1 };
+enum Limiter { MINMOD = 0, VANLEER = 1, MC = 2 };
+// Robustness variants of the Riemann step (readings R8b, R8c of DESIGN.md §14). PAPER.md:15
+// names only "the Roe's solver": flags = 0 is that plain solver and the default everywhere.
+enum RiemannFlags { ENTROPY_FIX = 1, HLLE_FALLBACK = 2 };
 
 // scalar helpers, overloaded for CountingReal in counting_real.hpp
 inline double o_sqrt(double x) { return std::sqrt(x); }
@@ -79,12 +82,17 @@ inline void phys_flux(const T U[5], const T W[5], int d, T F[5]) {
 //   zero when the signs differ or either difference is zero (sign test by comparison, not product);
 //   MinMod:   sign(dL) * min(|dL|, |dR|)
 //   van Leer: 2 dL dR / (dL + dR)               (harmonic mean)
+//   MC:       sign(dL) * min(2|dL|, 2|dR|, |dL + dR| / 2)   (monotonized central)
 template <class T>
 inline T limited_slope(T dL, T dR, int limiter) {
   const bool same_sign = (o_value(dL) > 0.0 && o_value(dR) > 0.0) || (o_value(dL) < 0.0 && o_value(dR) < 0.0);
   if (!same_sign) return T(0.0);
   if (limiter == MINMOD) {
     const T m = o_min(o_abs(dL), o_abs(dR));
+    return o_value(dL) > 0.0 ? m : -m;
+  }
+  if (limiter == MC) {
+    const T m = o_min(o_min(T(2.0) * o_abs(dL), T(2.0) * o_abs(dR)), T(0.5) * o_abs(dL + dR));
     return o_value(dL) > 0.0 ? m : -m;
   }
   return T(2.0) * dL * dR / (dL + dR);
@@ -148,8 +156,18 @@ inline void roe_decompose(const T UL[5], const T UR[5], T gamma, int d, RoeDecom
 
 // O5.  F = 1/2 [F(UL) + F(UR)] - 1/2 sum_i alpha_i |lambda_i| K_i, no entropy fix (R8); returned in
 // the global component order (rho, mx, my, mz, E), flux density along +axis d.
+// flags (default 0 = the plain solver above, readings R8b / R8c):
+//   ENTROPY_FIX   Harten & Hyman's fix of the two acoustic waves: with lambda_L, lambda_R the wave's speed u -+ a in the
+//                 states on its two sides (the outer state and the intermediate state U*_L = UL + alpha_1 K_1, resp.
+//                 U*_R = UR - alpha_5 K_5) and delta = max(0, lambda~ - lambda_L, lambda_R - lambda~), |lambda~| is
+//                 replaced by (lambda~^2 / delta + delta) / 2 wherever |lambda~| < delta, i.e. only inside a
+//                 transonic expansion, where plain Roe admits an expansion shock.
+//   HLLE_FALLBACK if either intermediate state of the linearisation, U*_L = UL + alpha_1 K_1 or U*_R = UR - alpha_5 K_5,
+//                 is non-physical (rho* <= 0 or 2 rho* E* <= |m*|^2), the flux is Einfeldt's HLLE flux
+//                 (b+ F_L - b- F_R + b+ b- (UR - UL)) / (b+ - b-), b- = min(u_L - a_L, u~ - a~, 0),
+//                 b+ = max(u_R + a_R, u~ + a~, 0), which is positivity preserving.
 template <class T>
-inline void roe_flux(const T UL[5], const T UR[5], T gamma, int d, T F[5]) {
+inline void roe_flux(const T UL[5], const T UR[5], T gamma, int d, T F[5], int flags = 0, bool* used_hlle = nullptr) {
   const int n = d, t1 = (d + 1) % 3, t2 = (d + 2) % 3;
   const int to_global[5] = {0, 1 + n, 1 + t1, 1 + t2, 4};
   RoeDecomp<T> R;
@@ -157,12 +175,66 @@ inline void roe_flux(const T UL[5], const T UR[5], T gamma, int d, T F[5]) {
   T FL[5], FR[5];
   phys_flux(UL, R.WL, d, FL);
   phys_flux(UR, R.WR, d, FR);
+  if (used_hlle) *used_hlle = false;
+  T absl1 = o_abs(R.lambda[0]), absl5 = o_abs(R.lambda[4]);
+  if (flags != 0) {
+    const T aL = o_sqrt(gamma * R.WL[4] / R.WL[0]), aR = o_sqrt(gamma * R.WR[4] / R.WR[0]);
+    const T uL = R.WL[1 + n], uR = R.WR[1 + n];
+    if (flags & HLLE_FALLBACK) {
+      // intermediate states in the rotated order (rho, m_n, m_t1, m_t2, E)
+      bool bad = false;
+      for (int side = 0; side < 2; ++side) {
+        const T* U = side == 0 ? UL : UR;
+        const T al = side == 0 ? R.alpha[0] : -R.alpha[4];
+        const T* K = side == 0 ? R.K[0] : R.K[4];
+        const T rs = U[0] + al * K[0];
+        const T mn = U[1 + n] + al * K[1], ma = U[1 + t1] + al * K[2], mb = U[1 + t2] + al * K[3];
+        const T Es = U[4] + al * K[4];
+        const T m2 = mn * mn + ma * ma + mb * mb;
+        if (!(o_value(rs) > 0.0 && o_value(T(2.0) * rs * Es) > o_value(m2))) bad = true;
+      }
+      if (bad) {
+        T bm = o_min(uL - aL, R.lambda[0]);
+        bm = o_min(bm, T(0.0));
+        T bp = -o_min(-(uR + aR), -R.lambda[4]);
+        bp = -o_min(-bp, T(0.0));
+        const T inv = T(1.0) / (bp - bm);
+        for (int q = 0; q < 5; ++q) F[q] = ((bp * FL[q] - bm * FR[q]) + (bp * bm) * (UR[q] - UL[q])) * inv;
+        if (used_hlle) *used_hlle = true;
+        return;
+      }
+    }
+    if (flags & ENTROPY_FIX) {
+      // speed of the acoustic wave on its two sides: in the outer state and in the intermediate state next to it
+      // (U*_L = UL + alpha_1 K_1 right of wave 1, U*_R = UR - alpha_5 K_5 left of wave 5); a non-physical
+      // intermediate state leaves the wave unfixed
+      for (int wave = 0; wave < 2; ++wave) {
+        const T* U = wave == 0 ? UL : UR;
+        const T al = wave == 0 ? R.alpha[0] : -R.alpha[4];
+        const T* K = wave == 0 ? R.K[0] : R.K[4];
+        const T sgn = wave == 0 ? T(-1.0) : T(1.0);
+        const T rs = U[0] + al * K[0];
+        const T mn = U[1 + n] + al * K[1], ma = U[1 + t1] + al * K[2], mb = U[1 + t2] + al * K[3];
+        const T Es = U[4] + al * K[4];
+        const T ps = (gamma - T(1.0)) * (Es - T(0.5) * (mn * mn + ma * ma + mb * mb) / rs);
+        if (!(o_value(rs) > 0.0 && o_value(ps) > 0.0)) continue;
+        const T lam_star = mn / rs + sgn * o_sqrt(gamma * ps / rs);
+        const T lam_out = (wave == 0 ? uL : uR) + sgn * (wave == 0 ? aL : aR);
+        const T lamL = wave == 0 ? lam_out : lam_star, lamR = wave == 0 ? lam_star : lam_out;
+        const T lam = wave == 0 ? R.lambda[0] : R.lambda[4];
+        T delta = -o_min(-(lam - lamL), -(lamR - lam));   // max of the two
+        delta = -o_min(-delta, T(0.0));                   // max(0, .)
+        T& absl = wave == 0 ? absl1 : absl5;
+        if (o_value(absl) < o_value(delta)) absl = T(0.5) * (lam * lam / delta + delta);
+      }
+    }
+  }
   // c_i = alpha_i |lambda_i|
-  const T c1 = R.alpha[0] * o_abs(R.lambda[0]);
+  const T c1 = R.alpha[0] * absl1;
   const T c2 = R.alpha[1] * o_abs(R.lambda[1]);
   const T c3 = R.alpha[2] * o_abs(R.lambda[2]);
   const T c4 = R.alpha[3] * o_abs(R.lambda[3]);
-  const T c5 = R.alpha[4] * o_abs(R.lambda[4]);
+  const T c5 = R.alpha[4] * absl5;
   // D = sum_i c_i K_i, component by component in the rotated order. Waves 1 and 5 are paired first so
   // that a mirror reflection reproduces the same bits (R21); structural 0/1 eigenvector entries
   // (K1[0]=K2[0]=K5[0]=1, K3[2]=K4[3]=1, the zeros of K3, K4) are written out, not multiplied.
@@ -189,12 +261,16 @@ inline void roe_flux(const T UL[5], const T UR[5], T gamma, int d, T F[5]) {
 //   margin same shape (nullable): min over the six predicted face states of
 //          (2 rho E - |m|^2) / (2 rho E), i.e. internal/total energy of the worst face state; it is a
 //          diagnostic for the parity harness (cells with |margin| ~ eps can flip in fp32), not used here.
+//   flags: RiemannFlags for O5 (default 0 = plain Roe).
+//   midflux (nullable): the fluxes on the three MID-planes of the box (the faces at index n/2 - 1/2 along each axis,
+//          between the two halves a group of 2 x 2 x 2 patches consists of; reading R12b): [3][5][.][.] in the
+//          in-face layout of the outer faces of the same axis, x mid-plane first. Needs even nx, ny, nz.
 // A patch group is the special case nx = ny = nz = N (O8: the per-group and global forms are the same text).
 struct StepStats { unsigned long long guard_cells = 0, nonpositive_out = 0; };
 
 template <class T>
 StepStats step_box(const T* U_in, int nx, int ny, int nz, int g, T dt, T dx, T gamma, int limiter,
-                   T* U_out, T* bflux, unsigned char* guard, double* margin) {
+                   T* U_out, T* bflux, unsigned char* guard, double* margin, int flags = 0, T* midflux = nullptr) {
   StepStats stats;
   const int sx = nx + 2 * g, sy = ny + 2 * g, sz = nz + 2 * g;
   const size_t plane = (size_t)sx * sy, vol = plane * sz;
@@ -317,7 +393,7 @@ StepStats step_box(const T* U_in, int nx, int ny, int nz, int g, T dt, T dx, T g
             UL[q] = ub(i - e[d][0], j - e[d][1], k - e[d][2], d, 1, q);  // left cell's '+' state
             UR[q] = ub(i, j, k, d, 0, q);                                // right cell's '-' state
           }
-          roe_flux(UL, UR, gamma, d, Ff);
+          roe_flux(UL, UR, gamma, d, Ff, flags);
           for (int q = 0; q < 5; ++q) fl(d, q, i, j, k) = Ff[q];
         }
 
@@ -355,6 +431,21 @@ StepStats step_box(const T* U_in, int nx, int ny, int nz, int g, T dt, T dx, T g
       for (int q = 0; q < 5; ++q)
         for (int j = 0; j < ny; ++j)
           for (int i = 0; i < nx; ++i) p[(((size_t)side * 5 + q) * ny + j) * nx + i] = fl(2, q, i, j, side ? nz : 0);
+  }
+  // O7b. mid-plane fluxes (R12b)
+  if (midflux) {
+    T* p = midflux;
+    for (int q = 0; q < 5; ++q)
+      for (int k = 0; k < nz; ++k)
+        for (int j = 0; j < ny; ++j) p[((size_t)q * nz + k) * ny + j] = fl(0, q, nx / 2, j, k);
+    p += (size_t)5 * nz * ny;
+    for (int q = 0; q < 5; ++q)
+      for (int k = 0; k < nz; ++k)
+        for (int i = 0; i < nx; ++i) p[((size_t)q * nz + k) * nx + i] = fl(1, q, i, ny / 2, k);
+    p += (size_t)5 * nz * nx;
+    for (int q = 0; q < 5; ++q)
+      for (int j = 0; j < ny; ++j)
+        for (int i = 0; i < nx; ++i) p[((size_t)q * ny + j) * nx + i] = fl(2, q, i, j, nz / 2);
   }
   return stats;
 }

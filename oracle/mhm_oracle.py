@@ -47,6 +47,11 @@ def lib():
         L.mhm_oracle_roe_decompose.argtypes = [_dp, _dp, C.c_double, C.c_int, _dp, _dp, _dp]
         L.mhm_oracle_count_flops.argtypes = [_dp, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
                                              _u64p]
+        L.mhm_oracle_step_groups_ex.restype = C.c_int
+        L.mhm_oracle_step_groups_ex.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
+                                                C.c_int, C.c_int, _dp, _dp, _dp, _u8p, _u64p, C.c_int]
+        L.mhm_oracle_roe_flux_ex.restype = C.c_int
+        L.mhm_oracle_roe_flux_ex.argtypes = [_dp, _dp, C.c_double, C.c_int, C.c_int, _dp]
         _lib = L
     return _lib
 
@@ -78,6 +83,35 @@ def step_groups(U_in, N, ghost, dt, dx, gamma, limiter, want_bflux=True, want_gu
                                         _ptr(out, _dp), _ptr(bf, _dp), _ptr(gd, _u8p), _ptr(mg, _dp),
                                         _ptr(stats, _u64p), int(n_threads))
     return StepResult(out, bf, gd, mg, int(stats[0]), int(stats[1]), int(used))
+
+
+ENTROPY_FIX, HLLE_FALLBACK = 1, 2
+
+
+def step_groups_ex(U_in, N, ghost, dt, dx, gamma, limiter, flags=0, want_midflux=False, n_threads=0):
+    """step_groups with the robustness variants: limiter 2 = MC, flags = ENTROPY_FIX |
+    HLLE_FALLBACK, optional mid-plane fluxes [G][3][5][N][N]. Returns (StepResult, midflux or None)."""
+    U = np.ascontiguousarray(U_in, dtype=np.float64)
+    S = N + 2 * ghost
+    assert U.ndim == 5 and U.shape[1:] == (5, S, S, S), U.shape
+    G = U.shape[0]
+    out = np.empty((G, 5, N, N, N), dtype=np.float64)
+    bf = np.empty((G, 6, 5, N, N), dtype=np.float64)
+    mf = np.empty((G, 3, 5, N, N), dtype=np.float64) if want_midflux else None
+    gd = np.zeros((G, N + 2, N + 2, N + 2), dtype=np.uint8)
+    stats = np.zeros(2, dtype=np.uint64)
+    used = lib().mhm_oracle_step_groups_ex(_ptr(U, _dp), G, N, ghost, float(dt), float(dx), float(gamma), int(limiter),
+                                           int(flags), _ptr(out, _dp), _ptr(bf, _dp), _ptr(mf, _dp), _ptr(gd, _u8p),
+                                           _ptr(stats, _u64p), int(n_threads))
+    return StepResult(out, bf, gd, None, int(stats[0]), int(stats[1]), int(used)), mf
+
+
+def roe_flux_ex(UL, UR, gamma, d, flags):
+    """Roe flux with RiemannFlags; returns (F, used_hlle)."""
+    F = np.empty(5)
+    h = lib().mhm_oracle_roe_flux_ex(_ptr(_vec5(UL), _dp), _ptr(_vec5(UR), _dp), float(gamma), int(d), int(flags),
+                                     _ptr(F, _dp))
+    return F, bool(h)
 
 
 def step_box(U_in, ghost, dt, dx, gamma, limiter):

@@ -49,6 +49,37 @@ int mhm_oracle_step_groups(const double* U_in, int n_groups, int N, int ghost, d
   return used < n_groups ? used : (n_groups > 0 ? n_groups : 1);
 }
 
+// The same with the robustness variants: flags = RiemannFlags, midflux [n_groups][3][5][N][N] or NULL.
+int mhm_oracle_step_groups_ex(const double* U_in, int n_groups, int N, int ghost, double dt, double dx, double gamma,
+                              int limiter, int flags, double* U_out, double* bflux, double* midflux,
+                              unsigned char* guard, unsigned long long* stats_out, int n_threads) {
+  const size_t S = (size_t)N + 2 * ghost;
+  const size_t in_sz = 5 * S * S * S, out_sz = (size_t)5 * N * N * N, bf_sz = (size_t)30 * N * N, mf_sz = (size_t)15 * N * N;
+  const size_t g_sz = (size_t)(N + 2) * (N + 2) * (N + 2);
+  unsigned long long gc = 0, npo = 0;
+  int used = 1;
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+  used = omp_get_max_threads();
+#pragma omp parallel for schedule(dynamic, 1) reduction(+ : gc, npo)
+#endif
+  for (int g = 0; g < n_groups; ++g) {
+    StepStats st = step_box<double>(U_in + g * in_sz, N, N, N, ghost, dt, dx, gamma, limiter, U_out + g * out_sz,
+                                    bflux ? bflux + g * bf_sz : nullptr, guard ? guard + g * g_sz : nullptr, nullptr,
+                                    flags, midflux ? midflux + g * mf_sz : nullptr);
+    gc += st.guard_cells;
+    npo += st.nonpositive_out;
+  }
+  if (stats_out) { stats_out[0] = gc; stats_out[1] = npo; }
+  return used < n_groups ? used : (n_groups > 0 ? n_groups : 1);
+}
+
+int mhm_oracle_roe_flux_ex(const double* UL, const double* UR, double gamma, int d, int flags, double* F) {
+  bool hlle = false;
+  roe_flux<double>(UL, UR, gamma, d, F, flags, &hlle);
+  return hlle ? 1 : 0;
+}
+
 // One global box (O8): U_in [5][nz+2g][ny+2g][nx+2g] -> U_out [5][nz][ny][nx]. Serial.
 void mhm_oracle_step_box(const double* U_in, int nx, int ny, int nz, int ghost, double dt, double dx, double gamma,
                          int limiter, double* U_out, double* bflux, unsigned char* guard, double* margin,
