@@ -32,7 +32,7 @@
  *                   normal) of (rho, mx, my, mz, E), exactly the value used in the update.
  * Ownership: the caller owns every buffer; the library never allocates, frees or keeps them. U_in is
  * read-only; outputs must not alias U_in. Device pointers must be 16-byte aligned.
- * Equation of state: ideal gas, E = P/(gamma-1) + rho |v|^2 / 2.  limiter: 0 = MinMod, 1 = van Leer.
+ * Equation of state: ideal gas, E = P/(gamma-1) + rho |v|^2 / 2.  limiter: 0 = MinMod, 1 = van Leer, 2 = MC.
  */
 #ifndef GAMER_HYDRO_H
 #define GAMER_HYDRO_H
@@ -52,7 +52,12 @@ enum {
   GAMER_HYDRO_NOT_SM100 = 4    /* the device is not compute capability 10.x */
 };
 
-enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1 };
+enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1, GAMER_HYDRO_MC = 2 /* monotonized central, R3b */ };
+
+/* Riemann-solver flags of gamer_hydro_step_ex (PAPER.md:15 names only "the Roe's solver", which
+ * is flags = 0): Harten & Hyman's entropy fix of the acoustic waves; Einfeldt's HLLE flux wherever an intermediate
+ * state of Roe's linearisation is non-physical. Readings R8b / R8c of DESIGN.md §14. */
+enum { GAMER_HYDRO_FLAG_ENTROPY_FIX = 1, GAMER_HYDRO_FLAG_HLLE_FALLBACK = 2 };
 
 /* kernel selection for gamer_hydro_set_path: AUTO picks FUSED when N == 16, else GENERIC. FUSED is the
  * performance path (fp32: one column per thread, the two lanes of every packed f32x2 instruction carry two
@@ -89,6 +94,20 @@ int gamer_hydro_step(const float* U_in_with_ghosts, float* U_out, float* boundar
 /* Same step in fp64 (parity target 1e-11 against the fp64 oracle). */
 int gamer_hydro_step_f64(const double* U_in_with_ghosts, double* U_out, double* boundary_fluxes, int n_groups,
                          int N, int ghost, double dt, double dx, double gamma, int limiter, cudaStream_t stream);
+
+/* The step with the robustness variants of SURVEY.md §8(f) rank 4: `flags` = GAMER_HYDRO_FLAG_* bits,
+ * and midplane_fluxes (DEVICE, may be NULL) = real[n_groups][3][5][N][N], the Roe fluxes on the three MID-planes of each
+ * group (the faces at index N/2 - 1/2 along x, y, z — the internal patch boundaries of a group of 2 x 2 x 2 patches, which
+ * the AMR flux fix-up needs beside the outer faces), each in the in-face layout of the outer faces of the same axis; N
+ * must be even. With flags = 0 and midplane_fluxes = NULL this is gamer_hydro_step (same kernels, same bits); otherwise
+ * the step runs in the scalar fused kernel (N = 16) or the shape-generic kernels. Other arguments, errors and
+ * execution semantics as gamer_hydro_step. */
+int gamer_hydro_step_ex(const float* U_in_with_ghosts, float* U_out, float* boundary_fluxes, float* midplane_fluxes,
+                        int n_groups, int N, int ghost, float dt, float dx, float gamma, int limiter, int flags,
+                        cudaStream_t stream);
+int gamer_hydro_step_ex_f64(const double* U_in_with_ghosts, double* U_out, double* boundary_fluxes,
+                            double* midplane_fluxes, int n_groups, int N, int ghost, double dt, double dx, double gamma,
+                            int limiter, int flags, cudaStream_t stream);
 
 /* Same fp32 step with HOST buffers (pinned memory recommended; pageable works but serialises the copies).
  * The batch is streamed through the device in chunks: H2D copy, kernel and D2H copy of consecutive chunks

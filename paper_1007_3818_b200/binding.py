@@ -14,13 +14,14 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _LIB_PATH = os.path.join(_HERE, "libgamer_hydro.so")
 _lib = None
 
-MINMOD, VANLEER = 0, 1
+MINMOD, VANLEER, MC = 0, 1, 2
+FLAG_ENTROPY_FIX, FLAG_HLLE_FALLBACK = 1, 2
 PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_DUO = 0, 1, 2, 3, 4
 
 EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
            "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance",
-           "gamer_hydro_step_grid", "gamer_hydro_set_guard_map", "gamer_rtvd_step"]
+           "gamer_hydro_step_grid", "gamer_hydro_set_guard_map", "gamer_rtvd_step", "gamer_hydro_step_ex", "gamer_hydro_step_ex_f64"]
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
@@ -50,6 +51,8 @@ def lib():
         L.gamer_hydro_advance.argtypes = [vp, vp, vp, i, i, i, i, i, i, i, i, i, f, f, f, i, vp, vp]
         L.gamer_hydro_set_guard_map.argtypes = [vp]
         L.gamer_rtvd_step.argtypes = [vp, vp, i, i, i, f, f, f, i, vp]
+        L.gamer_hydro_step_ex.argtypes = [vp, vp, vp, vp, i, i, i, f, f, f, i, i, vp]
+        L.gamer_hydro_step_ex_f64.argtypes = [vp, vp, vp, vp, i, i, i, d, d, d, i, i, vp]
         L.gamer_hydro_launch_count.restype = C.c_ulonglong
         L.gamer_hydro_strerror.restype = C.c_char_p
         L.gamer_hydro_strerror.argtypes = [i]
@@ -206,6 +209,42 @@ def gamer_hydro_status():
 
 def gamer_hydro_set_path(path):
     _check(lib().gamer_hydro_set_path(int(path)))
+
+
+def _step_ex(fn, dtype, U_in, U_out, boundary_fluxes, midplane_fluxes, N, ghost, dt, dx, gamma, limiter, flags, stream):
+    G = _shapes(U_in, N, ghost)
+    if U_out is None:
+        U_out = torch.empty((G, 5, N, N, N), dtype=dtype, device=U_in.device)
+    want = {"U_out": (U_out, (G, 5, N, N, N)), "boundary_fluxes": (boundary_fluxes, (G, 6, 5, N, N)),
+            "midplane_fluxes": (midplane_fluxes, (G, 3, 5, N, N))}
+    for name, (x, shape) in want.items():
+        if x is None:
+            continue
+        if not (x.is_cuda and x.dtype == dtype and x.is_contiguous() and x.device == U_in.device):
+            raise GamerHydroError("%s must be a contiguous CUDA tensor of dtype %s on the device of U_in" % (name, dtype))
+        if tuple(x.shape) != shape:
+            raise GamerHydroError("%s must have shape %s, got %s" % (name, shape, tuple(x.shape)))
+    if not (U_in.is_cuda and U_in.dtype == dtype and U_in.is_contiguous()):
+        raise GamerHydroError("U_in must be a contiguous CUDA tensor of dtype %s" % dtype)
+    ptr = lambda x: x.data_ptr() if x is not None else None
+    _check(fn(U_in.data_ptr(), U_out.data_ptr(), ptr(boundary_fluxes), ptr(midplane_fluxes), G, N, ghost, dt, dx, gamma,
+              int(limiter), int(flags), _stream_ptr(stream)))
+    return U_out
+
+
+def gamer_hydro_step_ex(U_in_with_ghosts, U_out, boundary_fluxes, midplane_fluxes, n_groups=None, N=16, ghost=2, dt=None,
+                        dx=None, gamma=5.0 / 3.0, limiter=MINMOD, flags=0, stream=None):
+    """fp32 step with the robustness variants (MC limiter via `limiter`, FLAG_* bits, mid-plane fluxes [G][3][5][N][N])."""
+    assert n_groups is None or n_groups == U_in_with_ghosts.shape[0]
+    return _step_ex(lib().gamer_hydro_step_ex, torch.float32, U_in_with_ghosts, U_out, boundary_fluxes, midplane_fluxes,
+                    N, ghost, dt, dx, gamma, limiter, flags, stream)
+
+
+def gamer_hydro_step_ex_f64(U_in_with_ghosts, U_out, boundary_fluxes, midplane_fluxes, n_groups=None, N=16, ghost=2,
+                            dt=None, dx=None, gamma=5.0 / 3.0, limiter=MINMOD, flags=0, stream=None):
+    assert n_groups is None or n_groups == U_in_with_ghosts.shape[0]
+    return _step_ex(lib().gamer_hydro_step_ex_f64, torch.float64, U_in_with_ghosts, U_out, boundary_fluxes,
+                    midplane_fluxes, N, ghost, dt, dx, gamma, limiter, flags, stream)
 
 
 def gamer_rtvd_step(U_in_with_ghosts, U_out, n_groups=None, N=16, ghost=3, dt=None, dx=None, gamma=5.0 / 3.0, sweep=0,

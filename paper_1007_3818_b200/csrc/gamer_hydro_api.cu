@@ -74,7 +74,9 @@ int cuda_fail(cudaError_t e, const char* what) {
 
 template <class R, int LIM, bool Fast>
 int set_fused_attr() {
-  CK(cudaFuncSetAttribute(gh::fused_kernel<R, LIM, Fast>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  CK(cudaFuncSetAttribute(gh::fused_kernel<R, LIM, Fast, false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                          gh::FusedSmem<R>::total));
+  CK(cudaFuncSetAttribute(gh::fused_kernel<R, LIM, Fast, true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                           gh::FusedSmem<R>::total));
   return 0;
 }
@@ -98,14 +100,19 @@ int init_locked(int device) {
   int rc;
   if ((rc = set_fused_attr<float, 0, true>())) return rc;
   if ((rc = set_fused_attr<float, 1, true>())) return rc;
+  if ((rc = set_fused_attr<float, 2, true>())) return rc;
   if ((rc = set_fused_attr<double, 0, false>())) return rc;
   if ((rc = set_fused_attr<double, 1, false>())) return rc;
+  if ((rc = set_fused_attr<double, 2, false>())) return rc;
   CK(cudaFuncSetAttribute(gh::zpair_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::ZSmem::total));
   CK(cudaFuncSetAttribute(gh::zpair_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::ZSmem::total));
+  CK(cudaFuncSetAttribute(gh::zpair_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::ZSmem::total));
   CK(cudaFuncSetAttribute(gh::duo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
+  CK(cudaFuncSetAttribute(gh::duo_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_halo_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::duo_halo_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
+  CK(cudaFuncSetAttribute(gh::duo_halo_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::DHALVES * gh::DuoSmem::total_padded));
   CK(cudaFuncSetAttribute(gh::rtvd_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::RtvdSmem::total));
   CK(cudaFuncSetAttribute(gh::rtvd_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, gh::RtvdSmem::total));
   void* fn = nullptr;
@@ -155,7 +162,8 @@ int validate(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, 
   if (n_groups < 0 || N < 1 || ghost < 2) return GAMER_HYDRO_INVALID_ARG;
   if (!(dt > R(0)) || !(dx > R(0)) || !isfinite((double)dt) || !isfinite((double)dx)) return GAMER_HYDRO_INVALID_ARG;
   if (!(gamma > R(1)) || !isfinite((double)gamma)) return GAMER_HYDRO_INVALID_ARG;
-  if (limiter != GAMER_HYDRO_MINMOD && limiter != GAMER_HYDRO_VANLEER) return GAMER_HYDRO_INVALID_ARG;
+  if (limiter != GAMER_HYDRO_MINMOD && limiter != GAMER_HYDRO_VANLEER && limiter != GAMER_HYDRO_MC)
+    return GAMER_HYDRO_INVALID_ARG;
   if (n_groups == 0) return 0;
   if (!U_in || !U_out) return GAMER_HYDRO_INVALID_ARG;
   if (((uintptr_t)U_in & 15) || ((uintptr_t)U_out & 15) || ((uintptr_t)bflux & 15)) return GAMER_HYDRO_INVALID_ARG;
@@ -191,9 +199,17 @@ int encode_plane_map(const R* U_in, int n_groups, int N, int ghost, CUtensorMap&
   return 0;
 }
 
+template <class R, int LIM, bool VAR>
+void launch_fused_one(int grid, int smem, cudaStream_t stream, const CUtensorMap& map, R* U_out, R* bflux, int n_groups,
+                      int goff, const gh::GasConst<R>& c, int flags, R* midflux) {
+  constexpr bool Fast = sizeof(R) == 4;
+  gh::fused_kernel<R, LIM, Fast, VAR><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, goff, c,
+                                                                         g_state.status, flags, midflux);
+}
+
 template <class R>
 int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma, int limiter,
-                 cudaStream_t stream) {
+                 cudaStream_t stream, int flags = 0, R* midflux = nullptr) {
   CUtensorMap map;
   int rc = encode_plane_map<R>(U_in, n_groups, N, ghost, map);
   if (rc) return rc;
@@ -203,13 +219,14 @@ int launch_fused(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int gho
   const int per_sm = (2 * smem + 2048 <= g_state.smem_per_sm && gh::FMINB >= 2) ? 2 : 1;
   const int resident = g_state.sm_count * per_sm;
   const int grid = n_groups < resident ? n_groups : resident;
-  constexpr bool Fast = sizeof(R) == 4;
-  if (limiter == 0)
-    gh::fused_kernel<R, 0, Fast><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c,
-                                                                   g_state.status);
-  else
-    gh::fused_kernel<R, 1, Fast><<<grid, gh::FNT, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c,
-                                                                   g_state.status);
+  const bool var = flags != 0 || midflux != nullptr;
+#define GH_FUSED(LIM)                                                                                               \
+  (var ? launch_fused_one<R, LIM, true>(grid, smem, stream, map, U_out, bflux, n_groups, ghost - 2, c, flags, midflux) \
+       : launch_fused_one<R, LIM, false>(grid, smem, stream, map, U_out, bflux, n_groups, ghost - 2, c, 0, nullptr))
+  if (limiter == 0) GH_FUSED(0);
+  else if (limiter == 1) GH_FUSED(1);
+  else GH_FUSED(2);
+#undef GH_FUSED
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   return 0;
@@ -229,12 +246,16 @@ int launch_duo(const float* U_in, float* U_out, float* bflux, int n_groups, int 
   if (halo) {
     if (limiter == 0)
       gh::duo_halo_kernel<0><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status, *halo);
-    else
+    else if (limiter == 1)
       gh::duo_halo_kernel<1><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status, *halo);
+    else
+      gh::duo_halo_kernel<2><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status, *halo);
   } else if (limiter == 0) {
     gh::duo_kernel<0><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
-  } else {
+  } else if (limiter == 1) {
     gh::duo_kernel<1><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  } else {
+    gh::duo_kernel<2><<<grid, threads, smem, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
   }
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
@@ -251,8 +272,10 @@ int launch_zpair(const float* U_in, float* U_out, float* bflux, int n_groups, in
   const int grid = n_groups < g_state.sm_count ? n_groups : g_state.sm_count;   // persistent: one CTA per SM
   if (limiter == 0)
     gh::zpair_kernel<0><<<grid, gh::ZNT, gh::ZSmem::total, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
-  else
+  else if (limiter == 1)
     gh::zpair_kernel<1><<<grid, gh::ZNT, gh::ZSmem::total, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
+  else
+    gh::zpair_kernel<2><<<grid, gh::ZNT, gh::ZSmem::total, stream>>>(map, U_out, bflux, n_groups, ghost - 2, c, g_state.status);
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   return 0;
@@ -260,7 +283,7 @@ int launch_zpair(const float* U_in, float* U_out, float* bflux, int n_groups, in
 
 template <class R>
 int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma,
-                   int limiter, cudaStream_t stream) {
+                   int limiter, cudaStream_t stream, int flags = 0, R* midflux = nullptr) {
   const int chunk = n_groups < kGenericChunk ? n_groups : kGenericChunk;
   int rc = ensure_scratch(generic_scratch_bytes<R>(chunk, N, ghost));
   if (rc) return rc;
@@ -280,9 +303,11 @@ int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int g
     R* bf = bflux ? bflux + (size_t)g0 * 30 * N * N : nullptr;
     const dim3 gp((unsigned)((ne + 127) / 128), ng), gf((unsigned)((nf + 127) / 128), ng),
         gu((unsigned)((nc + 127) / 128), ng);
+    R* mf = midflux ? midflux + (size_t)g0 * 15 * N * N : nullptr;
     if (limiter == 0) gh::predict_kernel<R, 0><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
-    else gh::predict_kernel<R, 1><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
-    gh::flux_kernel<R><<<gf, 128, 0, stream>>>(FS, FL, bf, sh, c);
+    else if (limiter == 1) gh::predict_kernel<R, 1><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
+    else gh::predict_kernel<R, 2><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
+    gh::flux_kernel<R><<<gf, 128, 0, stream>>>(FS, FL, bf, sh, c, flags, mf);
     gh::update_kernel<R><<<gu, 128, 0, stream>>>(in, FL, out, sh, c, g_state.status);
     g_launches.fetch_add(3);
   }
@@ -294,12 +319,19 @@ int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int g
 
 template <class R>
 int step_impl(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma, int limiter,
-              cudaStream_t stream) {
+              cudaStream_t stream, int flags = 0, R* midflux = nullptr) {
   int rc = validate<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter);
   if (rc) return rc;
+  if (flags < 0 || flags > 3 || ((uintptr_t)midflux & 15) || (midflux && (N & 1))) return GAMER_HYDRO_INVALID_ARG;
   if (n_groups == 0) return 0;
   if ((rc = ensure_init())) return rc;
   int path = g_state.path;
+  if (flags != 0 || midflux) {
+    // the robustness variants live in the scalar fused kernel (N = 16) and the generic kernels
+    if (path != GAMER_HYDRO_PATH_GENERIC && fused_supported<R>(N, ghost))
+      return launch_fused<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream, flags, midflux);
+    return launch_generic<R>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream, flags, midflux);
+  }
   if (path == GAMER_HYDRO_PATH_AUTO)
     path = fused_supported<R>(N, ghost) ? GAMER_HYDRO_PATH_FUSED : GAMER_HYDRO_PATH_GENERIC;
   if (path == GAMER_HYDRO_PATH_FUSED || path == GAMER_HYDRO_PATH_FUSED_SCALAR || path == GAMER_HYDRO_PATH_FUSED_DUO) {
@@ -434,6 +466,16 @@ int gamer_hydro_step(const float* U_in, float* U_out, float* bflux, int n_groups
 int gamer_hydro_step_f64(const double* U_in, double* U_out, double* bflux, int n_groups, int N, int ghost, double dt,
                          double dx, double gamma, int limiter, cudaStream_t stream) {
   return step_impl<double>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream);
+}
+
+int gamer_hydro_step_ex(const float* U_in, float* U_out, float* bflux, float* midflux, int n_groups, int N, int ghost,
+                        float dt, float dx, float gamma, int limiter, int flags, cudaStream_t stream) {
+  return step_impl<float>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream, flags, midflux);
+}
+
+int gamer_hydro_step_ex_f64(const double* U_in, double* U_out, double* bflux, double* midflux, int n_groups, int N,
+                            int ghost, double dt, double dx, double gamma, int limiter, int flags, cudaStream_t stream) {
+  return step_impl<double>(U_in, U_out, bflux, n_groups, N, ghost, dt, dx, gamma, limiter, stream, flags, midflux);
 }
 
 int gamer_hydro_max_speed(const void* U, int bytes_per_real, int n_groups, int N, int ghost, double gamma,

@@ -83,10 +83,20 @@ __device__ __forceinline__ float vanleer1(float a, float b, float p, float s) {
   const float q = (p + p) * rcp1(s);
   return p > 0.0f ? q : 0.0f;
 }
+// MC (monotonized central, R3b): sign(a) min(2|a|, 2|b|, |a + b| / 2) when the signs agree, else 0
+__device__ __forceinline__ float mc1(float a, float b, float s) {
+  float d;
+  asm("min.xorsign.abs.f32 %0, %1, %2;" : "=f"(d) : "f"(a), "f"(b));    // min(|a|,|b|), negative when the signs differ
+  const float m = fminf(d + d, 0.5f * fabsf(s));
+  return copysignf(fmaxf(m, 0.0f), a);
+}
 template <int LIM>
 __device__ __forceinline__ f2 limited_slope2(f2 a, f2 b) {
   if (LIM == 0) {
     return mk2(minmod1(lo(a), lo(b)), minmod1(hi(a), hi(b)));
+  } else if (LIM == 2) {
+    const f2 s = a + b;
+    return mk2(mc1(lo(a), lo(b), lo(s)), mc1(hi(a), hi(b), hi(s)));
   } else {
     const f2 p = a * b, s = a + b;
     return mk2(vanleer1(lo(a), lo(b), lo(p), lo(s)), vanleer1(hi(a), hi(b), hi(p), hi(s)));
@@ -199,6 +209,7 @@ __device__ __forceinline__ void sts2(float* p, f2 a) { *reinterpret_cast<unsigne
 template <int LIM>
 __device__ __forceinline__ float limited_slope1(float a, float b) {
   if (LIM == 0) return minmod1(a, b);
+  if (LIM == 2) return mc1(a, b, a + b);
   const float p = a * b, s = a + b;
   return vanleer1(a, b, p, s);
 }

@@ -81,10 +81,14 @@ __device__ __forceinline__ void tma_load_plane(uint32_t dst, const CUtensorMap* 
       : "memory");
 }
 
-template <class R, int LIM, bool Fast>
+// VAR = true: the robustness variants — run-time Riemann flags and the mid-plane flux array;
+// VAR = false is the plain kernel (flags fold to the literal 0, no extra argument is read).
+template <class R, int LIM, bool Fast, bool VAR = false>
 __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
     fused_kernel(const __grid_constant__ CUtensorMap in_map, R* __restrict__ U_out, R* __restrict__ bflux,
-                 int n_groups, int goff, GasConst<R> c, unsigned long long* __restrict__ status) {
+                 int n_groups, int goff, GasConst<R> c, unsigned long long* __restrict__ status, int flags_rt = 0,
+                 R* __restrict__ midflux = nullptr) {
+  const int flags = VAR ? flags_rt : 0;
   using SM = FusedSmem<R>;
   extern __shared__ __align__(128) unsigned char smem[];
   R* const wring = reinterpret_cast<R*>(smem + SM::off_w);
@@ -159,6 +163,7 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
     const int seq0 = it * FPLANES;  // sequence number of plane -2
     R* const outg = U_out + (size_t)g * (5 * FN * FN * FN);
     R* const bfg = bflux ? bflux + (size_t)g * (30 * FN * FN) : nullptr;
+    R* const mfg = (VAR && midflux) ? midflux + (size_t)g * (15 * FN * FN) : nullptr;
 
     R Wm[5], Wc[5], Wp[5], zplus[5], acc[5], Fzm[5];
     // prologue: planes -2 (own cell only) and -1 (own + extra, published for the x/y neighbours)
@@ -249,7 +254,11 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         R L[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) L[q] = xs[q * FNT + t_xl];
-        roe_flux<R, 0, Fast>(L, Wf[0][0], c, Fx);
+        roe_flux<R, 0, Fast>(L, Wf[0][0], c, Fx, flags);
+        if (VAR && mfg && i == FN / 2) {
+#pragma unroll
+          for (int q = 0; q < 5; ++q) mfg[(q * FN + k) * FN + j] = Fx[q];
+        }
 #pragma unroll
         for (int q = 0; q < 5; ++q) fxs[q * FNT + t] = Fx[q];
         if (bfg && (i == 0 || i == FN)) {
@@ -262,7 +271,11 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         R L[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) L[q] = ys[q * FNT + t_yl];
-        roe_flux<R, 1, Fast>(L, Wf[1][0], c, Fy);
+        roe_flux<R, 1, Fast>(L, Wf[1][0], c, Fy, flags);
+        if (VAR && mfg && j == FN / 2) {
+#pragma unroll
+          for (int q = 0; q < 5; ++q) mfg[((5 + q) * FN + k) * FN + i] = Fy[q];
+        }
 #pragma unroll
         for (int q = 0; q < 5; ++q) fys[q * FNT + t] = Fy[q];
         if (bfg && (j == 0 || j == FN)) {
@@ -272,7 +285,11 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         }
       }
       if (do_z) {
-        roe_flux<R, 2, Fast>(zplus, Wf[2][0], c, Fz);
+        roe_flux<R, 2, Fast>(zplus, Wf[2][0], c, Fz, flags);
+        if (VAR && mfg && k == FN / 2) {
+#pragma unroll
+          for (int q = 0; q < 5; ++q) mfg[((10 + q) * FN + j) * FN + i] = Fz[q];
+        }
         if (bfg && (k == 0 || k == FN)) {
           const int face = 4 + (k == FN);
 #pragma unroll

@@ -73,7 +73,8 @@ __global__ void __launch_bounds__(128) predict_kernel(const R* __restrict__ U_in
 
 template <class R, int n>
 __device__ __forceinline__ void flux_face(const R* __restrict__ FSg, R* __restrict__ FLg, R* __restrict__ bf,
-                                          const GenericShape& sh, const GasConst<R>& c, int i, int j, int k) {
+                                          const GenericShape& sh, const GasConst<R>& c, int i, int j, int k, int flags,
+                                          R* __restrict__ mf) {
   // face on the lower side of cell (i,j,k) along axis n; i in [0, N] along n
   const int E = sh.E, N = sh.N;
   const long long ev = (long long)E * E * E;
@@ -86,12 +87,17 @@ __device__ __forceinline__ void flux_face(const R* __restrict__ FSg, R* __restri
     L[q] = FSg[((n * 2 + 1) * 5 + q) * ev + el];
     Rt[q] = FSg[((n * 2 + 0) * 5 + q) * ev + er];
   }
-  roe_flux<R, n, false>(L, Rt, c, F);
+  roe_flux<R, n, false>(L, Rt, c, F, flags);
   const int fx = N + di, fy = N + dj;
   const long long nf = (long long)(N + 1) * N * N;
   const long long f = ((long long)k * fy + j) * fx + i;
 #pragma unroll
   for (int q = 0; q < 5; ++q) FLg[(n * 5 + q) * nf + f] = F[q];
+  if (mf && (n == 0 ? i : (n == 1 ? j : k)) == N / 2) {   // mid-plane fluxes (R12b), in-face layout of the outer faces
+    const int a = n == 2 ? j : k, b = n == 0 ? j : i;
+#pragma unroll
+    for (int q = 0; q < 5; ++q) mf[((n * 5 + q) * N + a) * N + b] = F[q];
+  }
   if (bf) {
     const int along = n == 0 ? i : (n == 1 ? j : k);
     if (along == 0 || along == N) {
@@ -106,7 +112,7 @@ __device__ __forceinline__ void flux_face(const R* __restrict__ FSg, R* __restri
 
 template <class R>
 __global__ void __launch_bounds__(128) flux_kernel(const R* __restrict__ FS, R* __restrict__ FL, R* __restrict__ bflux,
-                                                   GenericShape sh, GasConst<R> c) {
+                                                   GenericShape sh, GasConst<R> c, int flags, R* __restrict__ midflux) {
   const int N = sh.N;
   const long long nf = (long long)(N + 1) * N * N;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -116,11 +122,12 @@ __global__ void __launch_bounds__(128) flux_kernel(const R* __restrict__ FS, R* 
   const R* FSg = FS + (long long)blockIdx.y * sh.fs_stride;
   R* FLg = FL + (long long)blockIdx.y * sh.fl_stride;
   R* bf = bflux ? bflux + (long long)blockIdx.y * 30 * N * N : nullptr;
+  R* mf = midflux ? midflux + (long long)blockIdx.y * 15 * N * N : nullptr;
   const int fx = N + (n == 0), fy = N + (n == 1);
   const int i = (int)(f % fx), j = (int)((f / fx) % fy), k = (int)(f / ((long long)fx * fy));
-  if (n == 0) flux_face<R, 0>(FSg, FLg, bf, sh, c, i, j, k);
-  else if (n == 1) flux_face<R, 1>(FSg, FLg, bf, sh, c, i, j, k);
-  else flux_face<R, 2>(FSg, FLg, bf, sh, c, i, j, k);
+  if (n == 0) flux_face<R, 0>(FSg, FLg, bf, sh, c, i, j, k, flags, mf);
+  else if (n == 1) flux_face<R, 1>(FSg, FLg, bf, sh, c, i, j, k, flags, mf);
+  else flux_face<R, 2>(FSg, FLg, bf, sh, c, i, j, k, flags, mf);
 }
 
 template <class R>

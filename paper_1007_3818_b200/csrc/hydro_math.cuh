@@ -91,6 +91,10 @@ template <class R, int LIM, bool Fast>
 __device__ __forceinline__ R limited_slope(R dL, R dR) {
   if (LIM == 0) {
     return max_(R(0), min_(dL, dR)) + min_(R(0), max_(dL, dR));
+  } else if (LIM == 2) {
+    // MC (monotonized central, R3b): sign * min(2|dL|, 2|dR|, |dL + dR| / 2) when the signs agree
+    const R m = min_(min_(R(2) * abs_(dL), R(2) * abs_(dR)), R(0.5) * abs_(dL + dR));
+    return dL * dR > R(0) ? (dL > R(0) ? m : -m) : R(0);
   } else {
     const R p = dL * dR;
     const R s = dL + dR;
@@ -169,9 +173,11 @@ __device__ __forceinline__ bool predict_cell(const R Wc[5], const R Wm[3][5], co
 // Left/right states as primitives; returns the flux density along +axis n in global component order.
 // Wave strengths in the primitive-jump (Roe–Pike) form, which is algebraically identical to the
 // conserved-jump form the oracle uses:  a1,5 = (dp -+ rho~ a~ du)/(2 a~^2), a2 = drho - dp/a~^2,
-// a3,4 = rho~ dv, rho~ dw with rho~ = sqrt(rhoL rhoR). No entropy fix.
+// a3,4 = rho~ dv, rho~ dw with rho~ = sqrt(rhoL rhoR). flags = 0 (a literal in the default kernels, so the variant code
+// folds away): plain Roe, no entropy fix. Bit 0: Harten-Hyman entropy fix; bit 1: HLLE fallback when an intermediate
+// state of the linearisation is non-physical (readings R8b / R8c).
 template <class R, int n, bool Fast>
-__device__ __forceinline__ void roe_flux(const R L[5], const R Rt[5], const GasConst<R>& c, R F[5]) {
+__device__ __forceinline__ void roe_flux(const R L[5], const R Rt[5], const GasConst<R>& c, R F[5], int flags = 0) {
   constexpr int t1 = (n + 1) % 3, t2 = (n + 2) % 3;
   const R uL = L[1 + n], vL = L[1 + t1], wL = L[1 + t2];
   const R uR = Rt[1 + n], vR = Rt[1 + t1], wR = Rt[1 + t2];
@@ -194,9 +200,45 @@ __device__ __forceinline__ void roe_flux(const R L[5], const R Rt[5], const GasC
   const R t = dp * (rsa * rsa);
   const R s = (rt * du) * rsa;
   const R um = u - a, up = u + a;
+  const R mL = L[0] * uL, mR = Rt[0] * uR;
+  R absl1 = abs_(um), absl5 = abs_(up);
+  if (flags != 0) {
+    // intermediate states U*_L = UL + alpha_1 K_1, U*_R = UR - alpha_5 K_5 (rotated conserved components)
+    const R al1 = R(0.5) * (t - s), al5 = R(0.5) * (t + s), ua_ = u * a;
+    const R EL = L[0] * HL - L[4], ER = Rt[0] * HR - Rt[4];
+    const R r1 = L[0] + al1, n1 = mL + al1 * um, p1 = L[0] * vL + al1 * v, q1 = L[0] * wL + al1 * w, E1 = EL + al1 * (H - ua_);
+    const R r5 = Rt[0] - al5, n5 = mR - al5 * up, p5 = Rt[0] * vR - al5 * v, q5 = Rt[0] * wR - al5 * w, E5 = ER - al5 * (H + ua_);
+    const R k1 = n1 * n1 + p1 * p1 + q1 * q1, k5 = n5 * n5 + p5 * p5 + q5 * q5;
+    const bool ok1 = r1 > R(0) && R(2) * r1 * E1 > k1, ok5 = r5 > R(0) && R(2) * r5 * E5 > k5;
+    const R aL = sqrt(c.gamma * L[4] * (rsL * rsL)), aR = sqrt(c.gamma * Rt[4] * (rsR * rsR));
+    if ((flags & 2) && !(ok1 && ok5)) {
+      const R bm = min_(min_(uL - aL, um), R(0)), bp = max_(max_(uR + aR, up), R(0));
+      const R inv_b = R(1) / (bp - bm), bb = bp * bm;
+      F[0] = ((bp * mL - bm * mR) + bb * dr) * inv_b;
+      F[1 + n] = ((bp * (mL * uL + L[4]) - bm * (mR * uR + Rt[4])) + bb * (mR - mL)) * inv_b;
+      F[1 + t1] = ((bp * (mL * vL) - bm * (mR * vR)) + bb * (Rt[0] * vR - L[0] * vL)) * inv_b;
+      F[1 + t2] = ((bp * (mL * wL) - bm * (mR * wR)) + bb * (Rt[0] * wR - L[0] * wL)) * inv_b;
+      F[4] = ((bp * (mL * HL) - bm * (mR * HR)) + bb * (ER - EL)) * inv_b;
+      return;
+    }
+    if (flags & 1) {
+      if (ok1) {
+        const R ir = R(1) / r1;
+        const R ls = n1 * ir - sqrt(c.gamma * (c.g1 * (E1 - R(0.5) * k1 * ir)) * ir);   // u* - a* right of wave 1
+        const R delta = max_(R(0), max_(um - (uL - aL), ls - um));
+        if (absl1 < delta) absl1 = R(0.5) * (um * um / delta + delta);
+      }
+      if (ok5) {
+        const R ir = R(1) / r5;
+        const R ls = n5 * ir + sqrt(c.gamma * (c.g1 * (E5 - R(0.5) * k5 * ir)) * ir);   // u* + a* left of wave 5
+        const R delta = max_(R(0), max_(up - ls, (uR + aR) - up));
+        if (absl5 < delta) absl5 = R(0.5) * (up * up / delta + delta);
+      }
+    }
+  }
   // c_i = alpha_i |lambda_i|, with the overall factor 1/2 of the flux formula folded in
-  const R c1 = (R(0.25) * (t - s)) * abs_(um);
-  const R c5 = (R(0.25) * (t + s)) * abs_(up);
+  const R c1 = (R(0.25) * (t - s)) * absl1;
+  const R c5 = (R(0.25) * (t + s)) * absl5;
   const R au = R(0.5) * abs_(u);
   const R c2 = (dr - t) * au;
   const R c3 = (rt * dv) * au;
@@ -207,7 +249,6 @@ __device__ __forceinline__ void roe_flux(const R L[5], const R Rt[5], const GasC
   const R Dt2 = D0 * w + c4;
   const R ua = u * a;
   const R D4 = ((c1 * (H - ua) + c5 * (H + ua)) + c2 * hq) + (c3 * v + c4 * w);
-  const R mL = L[0] * uL, mR = Rt[0] * uR;
   F[0] = R(0.5) * (mL + mR) - D0;
   F[1 + n] = R(0.5) * ((mL * uL + L[4]) + (mR * uR + Rt[4])) - Dn;
   F[1 + t1] = R(0.5) * (mL * vL + mR * vR) - Dt1;

@@ -1,0 +1,102 @@
+"""GPU parity tests (-m gpu) of the robustness variants against the
+oracle's step_groups_ex: MC limiter on every kernel path, Harten-Hyman entropy fix and HLLE fallback (scalar fused and
+generic kernels), mid-plane fluxes; and that gamer_hydro_step_ex with everything off is gamer_hydro_step bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+import parity_util as pu
+import paper_1007_3818_b200 as gh
+from harness import metrics
+from harness import workloads as wl
+from oracle import mhm_oracle as O
+
+pytestmark = pytest.mark.gpu
+G = wl.GAMMA
+DEV = "cuda:0"
+PATHS = [gh.PATH_FUSED, gh.PATH_GENERIC, gh.PATH_FUSED_DUO, gh.PATH_FUSED_SCALAR]
+
+
+def run_ex(groups, dt, dx, limiter, flags, want_mid, path=gh.PATH_AUTO, N=16, ghost=2):
+    x = torch.from_numpy(np.ascontiguousarray(groups)).to(DEV)
+    n = x.shape[0]
+    out = torch.full((n, 5, N, N, N), float("nan"), dtype=x.dtype, device=DEV)
+    bf = torch.full((n, 6, 5, N, N), float("nan"), dtype=x.dtype, device=DEV)
+    mf = torch.full((n, 3, 5, N, N), float("nan"), dtype=x.dtype, device=DEV) if want_mid else None
+    fn = gh.gamer_hydro_step_ex if x.dtype == torch.float32 else gh.gamer_hydro_step_ex_f64
+    gh.gamer_hydro_set_path(path)
+    try:
+        fn(x, out, bf, mf, n, N, ghost, dt, dx, G, limiter, flags)
+        torch.cuda.synchronize()
+    finally:
+        gh.gamer_hydro_set_path(gh.PATH_AUTO)
+    return out.cpu().numpy(), bf.cpu().numpy(), (mf.cpu().numpy() if want_mid else None)
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-4), (np.float64, 1e-11)])
+@pytest.mark.parametrize("path", PATHS)
+def test_mc_limiter_on_every_kernel_path(path, dtype, tol):
+    g = wl.random_groups(4, seed=301, dtype=dtype)
+    dt, dx = (pu.f32(2e-3), pu.f32(1 / 16)) if dtype == np.float32 else (2e-3, 1 / 16)
+    out, bf, st = pu.run_gpu(g, dt, dx, G, gh.MC, path=path)
+    r, _ = O.step_groups_ex(g, 16, 2, dt, dx, G, gh.MC)
+    assert metrics.max_rel_err(out, r.U_out, G) <= tol
+    assert float(metrics.bflux_errors(bf, r.bflux, r.U_out, G).max()) <= 10 * tol
+    # and MC really is a different scheme from MinMod
+    r0 = O.step_groups(g, 16, 2, dt, dx, G, 0)
+    assert metrics.max_rel_err(r.U_out, r0.U_out, G) > 1e-4
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-4), (np.float64, 1e-11)])
+@pytest.mark.parametrize("path", [gh.PATH_AUTO, gh.PATH_GENERIC])
+@pytest.mark.parametrize("flags", [1, 2, 3])
+def test_entropy_fix_and_hlle_fallback_against_the_oracle(flags, path, dtype, tol):
+    """Supersonic random states (rms Mach 2): transonic expansions and non-physical intermediate states occur at many
+    faces, so both variants change the result; compared face flux by face flux and cell by cell."""
+    g = wl.random_groups(4, seed=302, mach=2.0, contrast=0.8, dtype=dtype)
+    dt, dx = (pu.f32(5e-4), pu.f32(1 / 16)) if dtype == np.float32 else (5e-4, 1 / 16)
+    out, bf, mf = run_ex(g, dt, dx, 1, flags, True, path=path)
+    r, mfo = O.step_groups_ex(g, 16, 2, dt, dx, G, 1, flags, want_midflux=True)
+    assert np.isfinite(out).all()
+    bad = np.zeros(g.shape[0], dtype=bool)
+    if dtype == np.float32 and (flags & 2):
+        # the HLLE switch is a discontinuous decision (like the guard R7): in fp32 a face whose intermediate state is
+        # marginal may take the other branch; such groups are set aside, and there must be few of them
+        e = metrics.cell_errors(out, r.U_out, G).reshape(g.shape[0], -1).max(axis=1)
+        bad = e > tol
+        assert bad.sum() <= 1, e
+    assert metrics.max_rel_err(out[~bad], r.U_out[~bad], G) <= tol
+    assert float(metrics.bflux_errors(bf[~bad], r.bflux[~bad], r.U_out[~bad], G).max()) <= 10 * tol
+    plain = O.step_groups(g, 16, 2, dt, dx, G, 1)
+    assert metrics.max_rel_err(r.U_out, plain.U_out, G) > 1e-3          # the variant is active on this input
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-4), (np.float64, 1e-11)])
+@pytest.mark.parametrize("path,N,ghost", [(gh.PATH_AUTO, 16, 2), (gh.PATH_GENERIC, 16, 2), (gh.PATH_AUTO, 8, 3)])
+def test_midplane_fluxes(path, N, ghost, dtype, tol):
+    g = wl.random_groups(3, seed=303, N=N, ghost=ghost, dtype=dtype)
+    dt, dx = (pu.f32(2e-3), pu.f32(1 / N)) if dtype == np.float32 else (2e-3, 1 / N)
+    out, bf, mf = run_ex(g, dt, dx, 0, 0, True, path=path, N=N, ghost=ghost)
+    r, mfo = O.step_groups_ex(g, N, ghost, dt, dx, G, 0, 0, want_midflux=True)
+    assert metrics.max_rel_err(out, r.U_out, G) <= tol
+    # scale of a mid-plane flux: the flux scale of an adjacent cell (metrics.bflux_errors' scale, taken at the plane)
+    mid = N // 2
+    rho, E, a = metrics._scales(r.U_out, G)
+    for ax, sl in enumerate([np.s_[:, :, :, mid], np.s_[:, :, mid, :], np.s_[:, mid, :, :]]):
+        base = rho[sl] * a[sl]
+        sc = [base, base * a[sl], base * a[sl], base * a[sl], base * a[sl] * a[sl]]
+        for q in range(5):
+            assert np.abs(mf[:, ax, q] - mfo[:, ax, q]).max() <= 10 * tol * sc[q].max()
+            assert (np.abs(mf[:, ax, q] - mfo[:, ax, q]) / sc[q]).max() <= 10 * tol
+
+
+def test_step_ex_with_everything_off_is_the_plain_step_bit_for_bit():
+    g = wl.random_groups(5, seed=304)
+    dt, dx = pu.f32(2e-3), pu.f32(1 / 16)
+    a = pu.run_gpu(g, dt, dx, G, 1)
+    out, bf, _ = run_ex(g, dt, dx, 1, 0, False)
+    assert np.array_equal(out, a[0]) and np.array_equal(bf, a[1])
+    with pytest.raises(gh.GamerHydroError):
+        run_ex(g, dt, dx, 1, 4, False)                                   # unknown flag bit
+    with pytest.raises(gh.GamerHydroError):
+        pu.run_gpu(g, dt, dx, G, 3)                                      # unknown limiter
