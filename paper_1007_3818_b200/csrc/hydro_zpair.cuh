@@ -26,12 +26,17 @@
 //   P  slopes, face values, own-direction fluxes -> dU, the six predicted states, guard (reading R7);
 //      x+ / y+ states -> S[s&1];                                            arrive(S)
 //   Z  (interior) packed Roe solve at the two lower z faces of the pair (own registers only)
-//      wait(F of slot s-1)
-//   U  (interior) conservative update of pair s-1, U_out stores; (warp 9) boundary fluxes of pair s-1; TMA refill
-//      wait(S)   — also makes W[(s+1)&1] visible for the next slot
-//   R  packed Roe solves at the lower x and the lower y face of the pair -> F[s&1];   arrive(F)
-// Both barriers are split (mbarrier arrive by one elected lane per warp / try_wait): Z and U sit between arrive(S)
-// and wait(S), C, P and Z of the next slot between arrive(F) and wait(F).
+//      wait(S)
+//   R  packed Roe solves at the lower x and the lower y face of the pair -> F[s&1]
+//   U  (interior) conservative update of pair s-1 from F[(s-1)&1], U_out stores; (warp 9) boundary fluxes of pair s-1
+// ONE split barrier per slot (mbarrier, arrive by one elected lane per warp / try_wait): everything a warp publishes in
+// slot s — W[(s+1)&1] in C, S[s&1] in P, F[(s-1)&1] in the R of slot s-1 — is ordered before its arrive(S) of slot s;
+// a warp that has passed wait(S) of slot s therefore sees the states of pair s, the fluxes of pair s-1 and the
+// primitives of pair s+1, and knows that every warp has finished slot s-1 (so S[s&1], F[s&1] and W[(s+1)&1], last read
+// in slots s-2 / s-1, may be overwritten). Z sits between arrive and wait and absorbs the skew between warps. The TMA
+// producer refills a raw stage after wait(S) of slot s: the pairs <= s-2 are retired (last reader: the U of slot s-1).
+// (Tried and dropped, profiles/r2b_README.md: splitting the warps into two half-CTA sets that run half a slot apart —
+// the extra cross-set waits cost more than the overlap of P with Z / R / U gains.)
 // Follows PAPER.md:15 with the readings of DESIGN.md §3; shares no code with oracle/.
 #pragma once
 #include <cuda.h>
@@ -43,16 +48,9 @@
 
 namespace gh {
 
-#ifndef GH_ZNT
-#define GH_ZNT 320
-#endif
-constexpr int ZNT = GH_ZNT;         // threads per CTA: 8 interior warps + 2 ghost warps (320), or + 2 x 2 ghost warps that alternate slots (384)
-constexpr bool ZROT = ZNT == 384;
-constexpr int ZNW = ZNT / 32;       // warps (arrival count of the split barriers)
-#ifndef GH_ZNS
-#define GH_ZNS 5
-#endif
-constexpr int ZNS = GH_ZNS;         // raw ring depth in plane PAIRS
+constexpr int ZNT = 320;            // threads per CTA: 8 interior warps + 2 ghost warps
+constexpr int ZNW = ZNT / 32;       // warps (arrival count of the slot barrier)
+constexpr int ZNS = 6;              // raw ring depth in plane PAIRS (6 x 16 KB: the most that fits; 5 is 1.2 % slower)
 constexpr int ZSLOTS = 11;          // pipeline slots (= TMA loads) per group
 constexpr int ZWP = 21;             // row pitch of a primitive pair-plane in 8-byte elements (odd: the ghost columns read conflict-free)
 constexpr int ZWQ = FS * ZWP;       // elements per component
@@ -69,7 +67,7 @@ struct ZSmem {
   static constexpr int off_w = off_raw + ZNS * raw_stage_bytes;
   static constexpr int off_s = off_w + 2 * w_bytes;
   static constexpr int off_f = off_s + 2 * s_bytes;
-  static constexpr int off_bar = ((off_f + 2 * f_bytes + 15) / 16) * 16;  // ZNS full barriers, S, F
+  static constexpr int off_bar = ((off_f + 2 * f_bytes + 15) / 16) * 16;  // ZNS full barriers, S (even slots), S (odd slots)
   static constexpr int total = off_bar + (ZNS + 2) * 8;
 };
 static_assert(ZSmem::total <= 232448, "z-pair kernel: shared memory over the 227 KB limit");
@@ -190,12 +188,11 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   float* const fbase = reinterpret_cast<float*>(smem + SM::off_f);
   const uint32_t raw_base = smem_u32(smem + SM::off_raw);
   const uint32_t bar_base = smem_u32(smem + SM::off_bar);
-  const uint32_t s_bar = bar_base + 8 * ZNS, f_bar = s_bar + 8;
+  const uint32_t s_bar = bar_base + 8 * ZNS;   // the slot barrier, as an (even slot, odd slot) pair
 
   // ---- thread -> column (i, j); ghost lanes: rot = the normal is y
   const int t = (int)threadIdx.x, lane = t & 31;
-  const int role = t < 256 ? 0 : 1 + ((t >> 5) & 1);       // warp-uniform: warps 8, 10 upper ghosts, 9, 11 lower ghosts
-  const int duty_par = t >= 320 ? 1 : 0;                   // ghost warps 8, 9 work in the even slots, 10, 11 in the odd ones
+  const int role = t < 256 ? 0 : 1 + ((t >> 5) & 1);       // warp-uniform: warp 8 upper ghosts, warp 9 lower ghosts
   int i, j;
   bool rot = false;
   if (role == 0) { j = t >> 4; i = t & 15; }
@@ -234,7 +231,6 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   const bool producer = t == 288;
   if (producer) issue_upto(ZNS);
 
-  uint32_t s_phase = 0, f_phase = 1;   // the first wait(F) passes on the fresh barrier
   auto warp_arrive = [&](uint32_t bar) {
     __syncwarp();
     if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
@@ -270,13 +266,12 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
 #pragma unroll
     for (int q = 0; q < 5; ++q) az[q] = 0.0f;
   }
-  // interior: z+ state of the pair's upper plane (left state of the next pair's first z face), xy flux sums and
-  // z-flux differences of the pair awaiting its update
+  // interior: z+ state of the pair's upper plane (left state of the next pair's first z face) and the z-flux
+  // differences of the pair awaiting its update
   float Lz[6] = {1.0f, 1.0f, 1.0f, 1.0f, 1.0f, 1.0f};
-  f2 accxy[5];
   float dzlo[5], Fzh[5];
 #pragma unroll
-  for (int q = 0; q < 5; ++q) { accxy[q] = c.one; dzlo[q] = 0.0f; Fzh[q] = 0.0f; }
+  for (int q = 0; q < 5; ++q) { dzlo[q] = 0.0f; Fzh[q] = 0.0f; }
 
   // The slot body is written as straight-line PHASES (lambdas, inlined) so that each region between two barrier
   // operations is one basic block the scheduler can interleave: {C, P}, {Z, U}, {R, reload}. Slot-dependent special
@@ -425,8 +420,9 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
 #pragma unroll
       for (int q = 0; q < 5; ++q) {
         const f2 Uin = mk2(rawp[q * (2 * FS * FS)], rawp[q * (2 * FS * FS) + FS * FS]);
-        const f2 up = lds2(fx + 2 * q * ZNX + ix + 2) + lds2(fy + 2 * q * ZNY + iy + 2 * FN);
-        out[q] = fma2(c.lamn, (up - accxy[q]) + dzz[q], Uin);
+        const f2 dx = lds2(fx + 2 * q * ZNX + ix + 2) - lds2(fx + 2 * q * ZNX + ix);
+        const f2 dy = lds2(fy + 2 * q * ZNY + iy + 2 * FN) - lds2(fy + 2 * q * ZNY + iy);
+        out[q] = fma2(c.lamn, (dx + dy) + dzz[q], Uin);
       }
 #pragma unroll
       for (int q = 0; q < 5; ++q) {
@@ -475,7 +471,6 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
       for (int q = 0; q < 5; ++q) {
         sts2(fx + 2 * q * ZNX + ix, Fx[q]);
         sts2(fy + 2 * q * ZNY + iy, Fy[q]);
-        accxy[q] = Fx[q] + Fy[q];
       }
     } else if (role == 1) {
       // the face this ghost owns: x = 15.5 (column i = 16: left state SX[16 + 17 j], right state its x- state) or
@@ -510,71 +505,44 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
     const float* const fxp = fbase + (buf ^ 1) * (SM::f_bytes / 4);   // fluxes of slot s-1
     const float* const fyp = fxp + 10 * ZNX;
 
-    // the ghost columns are served by two pairs of warps in alternate slots (the four schedulers then carry the same
-    // load); a ghost warp keeps no state between its slots: it re-reads its column from the primitive pair-planes
-    const bool duty = !ZROT || role == 0 || ((s & 1) == duty_par);
-    auto wait_f = [&]() {
-      mbar_wait_sleep(f_bar, f_phase);       // every warp has finished slot s-1 (arrived at its end: long since)
-      f_phase ^= 1u;
+    const uint32_t sbar = s_bar + 8u * (uint32_t)(s & 1), spar = (uint32_t)(s >> 1) & 1u;   // barrier / parity of slot s
+    auto wait_s = [&]() {
+      mbar_wait_sleep(sbar, spar);           // see the header: states of pair s, fluxes of pair s-1, primitives of pair s+1
       if (producer) issue_upto(s - 1 + ZNS); // pairs <= s-2 are retired (their last reader is the update in slot s-1)
     };
-    auto wait_s = [&]() {
-      mbar_wait_sleep(s_bar, s_phase);       // x+ / y+ states of this pair and the primitives of pair s+1 are visible
-      s_phase ^= 1u;
-    };
-    if (duty) {
-      if (ZROT && role != 0) {
-        az[0] = w_nxt[w_own + 1];   // upper plane of pair s-1 (this warp's pair-plane of two slots ago, about to be overwritten)
-        az[1] = w_nxt[w_own + 2 * ZWQ + 1]; az[2] = w_nxt[w_own + 4 * ZWQ + 1];
-        az[3] = w_nxt[w_own + 6 * ZWQ + 1]; az[4] = w_nxt[w_own + 8 * ZWQ + 1];
-        load_own(w_cur, Wc);
+    float cz[5];
+    phaseC(w_nxt, cz);
+    if (gs >= 1 && gs <= 9) {
+      // ================= a full slot: the pair (2 gs - 3, 2 gs - 2) =================
+      St2 Sm1, Sm2, Szm, Szp;
+      phaseP(w_cur, sx, sy, cz, Sm1, Sm2, Szm, Szp);
+      warp_arrive(sbar);                    // everything the neighbours need from this warp is published
+      f2 dzz[5];
+      if (role == 0) phaseZ(Szm, Szp, dzz);
+      if (role == 0 && bfg && (gs == 1 || gs == 9)) {   // a5: faces -z (the upper face of plane -1) and +z (of plane 15)
+        float* p = bfg + (4 + (gs == 9)) * (5 * FN * FN) + j * FN + i;
 #pragma unroll
-        for (int q = 0; q < 5; ++q) az[q] = lo(Wc[q]) - az[q];
+        for (int q = 0; q < 5; ++q) p[q * (FN * FN)] = Fzh[q];
       }
-      float cz[5];
-      phaseC(w_nxt, cz);
-      if (gs >= 1 && gs <= 9) {
-        // ================= a full slot: the pair (2 gs - 3, 2 gs - 2) =================
-        St2 Sm1, Sm2, Szm, Szp;
-        phaseP(w_cur, sx, sy, cz, Sm1, Sm2, Szm, Szp);
-        warp_arrive(s_bar);                    // everything the neighbours need from this warp is published
-        wait_f();
-        f2 dzz[5];
-        if (role == 0) phaseZ(Szm, Szp, dzz);
-        if (gs >= 3) phaseU(T_{}, T_{}, fxp, fyp, outg, bfg, dzz);
-        else if (gs == 2) phaseU(F_{}, T_{}, fxp, fyp, outg, bfg, dzz);
-        if (role == 0 && bfg && (gs == 1 || gs == 9)) {   // a5: faces -z (the upper face of plane -1) and +z (of plane 15)
-          float* p = bfg + (4 + (gs == 9)) * (5 * FN * FN) + j * FN + i;
-#pragma unroll
-          for (int q = 0; q < 5; ++q) p[q * (FN * FN)] = Fzh[q];
-        }
-        wait_s();
-        phaseR(sx, sy, fx, fy, Sm1, Sm2);
-      } else {
-        // ================= a light slot: gs = 0 (planes -3, -2) converts the first pair, gs = 10 finishes the last =====
-        warp_arrive(s_bar);
-        wait_f();
-        if (gs == ZSLOTS - 1) {
-          f2 dzz[5];   // plane 16 gets no update; plane 15 needs the z difference it already has
-#pragma unroll
-          for (int q = 0; q < 5; ++q) dzz[q] = mk2(dzlo[q], 0.0f);
-          phaseU(T_{}, F_{}, fxp, fyp, outg, bfg, dzz);
-        }
-        wait_s();
-      }
-      // ---- next pair (interior): own column of W[(s+1)&1] (written by this thread in C), the z difference below it
-      if (!ZROT || role == 0) {
-        load_own(w_nxt, Wc);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) az[q] = cz[q];
-      }
-    } else {
-      skip_raw();
-      warp_arrive(s_bar);
-      wait_f();
       wait_s();
+      phaseR(sx, sy, fx, fy, Sm1, Sm2);
+      if (gs >= 3) phaseU(T_{}, T_{}, fxp, fyp, outg, bfg, dzz);
+      else if (gs == 2) phaseU(F_{}, T_{}, fxp, fyp, outg, bfg, dzz);
+    } else {
+      // ================= a light slot: gs = 0 (planes -3, -2) converts the first pair, gs = 10 finishes the last =====
+      warp_arrive(sbar);
+      wait_s();
+      if (gs == ZSLOTS - 1) {
+        f2 dzz[5];   // plane 16 gets no update; plane 15 needs the z difference it already has
+#pragma unroll
+        for (int q = 0; q < 5; ++q) dzz[q] = mk2(dzlo[q], 0.0f);
+        phaseU(T_{}, F_{}, fxp, fyp, outg, bfg, dzz);
+      }
     }
-    warp_arrive(f_bar);
+    // ---- next pair: own column of W[(s+1)&1] (written by this thread in C), the z difference below it
+    load_own(w_nxt, Wc);
+#pragma unroll
+    for (int q = 0; q < 5; ++q) az[q] = cz[q];
     if (++u_stage == ZNS) u_stage = 0;
     if (++gs == ZSLOTS) { gs = 0; g += (int)gridDim.x; }
   }
