@@ -46,6 +46,8 @@ RTVD_FLOPS_PER_CELL = 1279.0
 RTVD_BYTES_PER_CELL = (5 * 22 ** 3 + 5 * 16 ** 3) * 4 / 16 ** 3      # 72.0
 SM_COUNT, LANES, SM_MAX_GHZ = 148, 128, 1.965
 ALU_PEAK_TFLOPS = SM_COUNT * LANES * 2 * SM_MAX_GHZ / 1e3     # 74.45
+FP64_PEAK_TFLOPS = SM_COUNT * 64 * 2 * SM_MAX_GHZ / 1e3        # 37.22
+ISSUE_COST_PER_CELL = 960.0     # scheduler clocks per cell-update the MinMod z-pair kernel's instruction mix costs (profiles/r2b_README.md)
 
 
 def measured_hbm_peak():
@@ -355,11 +357,11 @@ def main():
     hbm_gbs = BYTES_PER_CELL * cells / (ms_launch * 1e-3) / 1e9
     traffic, traffic_src = None, None
     try:
-        with open(os.path.join(ROOT, "profiles", "r2_traffic_bytes_per_launch.txt")) as f:
+        with open(os.path.join(ROOT, "profiles", "r2b_traffic_bytes_per_launch.txt")) as f:
             tj = json.load(f)
             if tj.get("n_groups") == G and args.path in ("auto", "fused"):
                 traffic = tj["dram_bytes_read_plus_write"]
-                traffic_src = "ncu --set full capture, profiles/r2_traffic_bytes_per_launch.txt (commit %s)" % tj.get("commit")
+                traffic_src = "ncu --set full capture, profiles/r2b_traffic_bytes_per_launch.txt (commit %s)" % tj.get("commit")
     except Exception:
         pass
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
@@ -379,6 +381,16 @@ def main():
                         "peak_gbs": hbm_peak, "peak_source": hbm_src, "frac": hbm_gbs / hbm_peak},
                 "frac_of_binding_roofline_time": max(flops / (ALU_PEAK_TFLOPS * 1e12),
                                                      BYTES_PER_CELL * cells / (hbm_peak * 1e9)) / (ms_launch * 1e-3)}
+    if args.path in ("auto", "fused") and w.limiter == 0:
+        # what the step costs the warp schedulers (explanatory, not a roofline): scheduler clocks per cell-update of this
+        # run against the issue cost of the kernel's executed instruction mix (profiles/r2b_README.md: packed f32x2 = 2
+        # clocks, 3 with three distinct source pairs; measured by harness/issue_microbench.py)
+        clocks = ms_launch * 1e-3 * SM_MAX_GHZ * 1e9 * SM_COUNT * 4 * 32 / cells
+        roofline["issue"] = {"scheduler_clocks_per_cell_update": clocks,
+                             "issue_cost_of_instruction_mix": ISSUE_COST_PER_CELL,
+                             "frac_of_issue_bound": ISSUE_COST_PER_CELL / clocks,
+                             "clocks_at_target_frac": FLOPS_PER_CELL[0] / (2 * 0.60),
+                             "source": "profiles/r2b_README.md, harness/issue_microbench.py"}
 
     # ---- cpu_baseline: the oracle on a bounded sample of the same workload (+ parity spot-check)
     cpu = None
@@ -460,6 +472,37 @@ def main():
                              "hbm_frac": RTVD_BYTES_PER_CELL * c3 / (ms3 * 1e-3) / 1e9 / hbm_peak}}
         del g3, o3
 
+    # ---- the fp64 entry (the 1e-11 parity path) on the 256^3 box of the same recipe, with its own roofline
+    f64 = None
+    if not args.no_multistep and world == 1:
+        from harness import workloads as wl
+        w4 = wl.config_3_cosmo(min(args.box, 256), seed=args.seed)
+        g4 = torch.from_numpy(wl.cut_groups(w4.U, w4.bc, ghost=2).astype(np.float64)).to(dev)
+        n4 = g4.shape[0]
+        o4 = torch.empty((n4, 5, N, N, N), dtype=torch.float64, device=dev)
+        b4 = torch.empty((n4, 6, 5, N, N), dtype=torch.float64, device=dev)
+        dt4, dx4 = float(w4.dt()), float(w4.dx)
+        for s in range(3):
+            gh.gamer_hydro_step_f64(g4, o4, b4, n4, N, 2, dt4, dx4, w4.gamma, 0, stream=stream)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for s in range(10):
+            gh.gamer_hydro_step_f64(g4, o4, b4, n4, N, 2, dt4, dx4, w4.gamma, 0, stream=stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms4 = e0.elapsed_time(e1) / 10
+        c4 = n4 * N ** 3
+        tf4 = FLOPS_PER_CELL[0] * c4 / (ms4 * 1e-3) / 1e12
+        f64 = {"value": c4 / (ms4 * 1e-3), "unit": UNIT, "ms_per_step": ms4, "groups": n4, "dtype": "f64",
+               "api": "gamer_hydro_step_f64", "kernel": "gh::fused_kernel<double, MinMod>",
+               "roofline": {"bound": "alu (fp64)", "flops_per_cell_update": FLOPS_PER_CELL[0], "achieved": tf4,
+                            "peak": FP64_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": tf4 / FP64_PEAK_TFLOPS,
+                            "peak_derivation": "148 SM x 64 FP64 lanes x 2 FLOP x 1.965 GHz (DFMA rate measured by "
+                                               "harness/issue_microbench.py: 2 clocks per warp instruction and scheduler)",
+                            "hbm_frac": 2 * BYTES_PER_CELL * c4 / (ms4 * 1e-3) / 1e9 / hbm_peak}}
+        del g4, o4, b4
+
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": total_ms_max / args.steps, "higher_is_better": True,
            "scaling": args.scaling if world > 1 else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -472,7 +515,7 @@ def main():
                                      ("the one batch split into contiguous ranges" if args.scaling == "strong" and world > 1
                                       else "the full batch on every rank"),
                       "generation_seconds": gen_s, "dt": dt, "dx": dx, "kernel_path": args.path},
-           "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "multistep": multistep, "rtvd": rtvd,
+           "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "multistep": multistep, "rtvd": rtvd, "f64": f64,
            "gpu_launches": int(launches),
            "clocks": clocks, "ms_per_step_min": min(per_step), "ms_per_step_median": float(np.median(per_step)),
            "guard_cells_per_step": guard_cells / args.steps, "nonpositive_out_per_step": nonpos / args.steps,

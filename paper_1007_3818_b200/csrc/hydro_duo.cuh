@@ -42,16 +42,13 @@ __device__ __forceinline__ void set2(f2& d, float a, float b) {
   asm volatile("mov.b64 %0, {%1, %2};" : "+l"(d.v) : "f"(a), "f"(b));
 }
 
-// Exchange arrays hold, per quantity m, FNT (lo, hi) lane pairs. GH_SPLIT_EXCH = 1 (default): the two lanes in
-// separate FNT-word planes (two 32-bit stores, conflict-free reads); 0: pair-packed (one 64-bit store per pair, but the
-// 32-bit reads of one lane are 2-way bank-conflicted). Measured on the headline configuration: 4.901 vs 4.933 ms.
-#ifndef GH_SPLIT_EXCH
-#define GH_SPLIT_EXCH 1
-#endif
-__device__ __forceinline__ int ex_off(int slot, int lane) { return GH_SPLIT_EXCH ? lane * FNT + slot : 2 * slot + lane; }
+// Exchange arrays hold, per quantity m, FNT (lo, hi) lane pairs with the two lanes in separate FNT-word planes: two
+// 32-bit stores, conflict-free 32-bit reads (pair-packed 64-bit stores make the reads of one lane 2-way conflicted:
+// 4.933 against 4.901 ms on the headline configuration).
+__device__ __forceinline__ int ex_off(int slot, int lane) { return lane * FNT + slot; }
 __device__ __forceinline__ void ex_put(float* base /* + ex_off(t, 0) */, int m, f2 v) {
-  if (GH_SPLIT_EXCH) { base[m * (2 * FNT)] = lo(v); base[m * (2 * FNT) + FNT] = hi(v); }
-  else sts2(base + m * (2 * FNT), v);
+  base[m * (2 * FNT)] = lo(v);
+  base[m * (2 * FNT) + FNT] = hi(v);
 }
 
 // scalar state for the z-face solve

@@ -27,10 +27,7 @@ namespace gh {
 constexpr int FN = 16;              // interior cells per axis
 constexpr int FS = FN + 4;          // stored cells per axis that are read (2 ghost layers)
 constexpr int FNT = 320;            // threads per CTA
-#ifndef GH_FMINB
-#define GH_FMINB 2
-#endif
-constexpr int FMINB = GH_FMINB;     // resident CTAs per SM the kernel is compiled for
+constexpr int FMINB = 2;            // resident CTAs per SM the fp32 instantiation is compiled for
 constexpr int FPLANES = FN + 4;     // planes -2 .. 17 per group
 constexpr int FNSTAGE = 6;          // raw ring depth
 constexpr int WPITCH = 114;         // row pitch (reals) of the primitive plane: rows [r][q][c], 114 = 18 mod 32
@@ -48,7 +45,10 @@ struct FusedSmem {
   static constexpr int off_ys = off_xs + exch;
   static constexpr int off_fx = off_ys + exch;
   static constexpr int off_fy = off_fx + exch;
-  static constexpr int off_bar = ((off_fy + exch + 15) / 16) * 16;
+  static constexpr int off_zs = off_fy + exch;                        // the thread's own z+ state of the plane below (kept out of registers)
+  static constexpr int off_wm = off_zs + exch;                        // the thread's own primitives of the plane below
+  static constexpr int off_acc = off_wm + exch;                       // (xy flux differences - lower z flux) of the plane awaiting its update
+  static constexpr int off_bar = ((off_acc + exch + 15) / 16) * 16;
   static constexpr int total = off_bar + FNSTAGE * 8 + 16;
 };
 
@@ -96,6 +96,9 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
   R* const ys = reinterpret_cast<R*>(smem + SM::off_ys);
   R* const fxs = reinterpret_cast<R*>(smem + SM::off_fx);
   R* const fys = reinterpret_cast<R*>(smem + SM::off_fy);
+  R* const zs = reinterpret_cast<R*>(smem + SM::off_zs);
+  R* const wms = reinterpret_cast<R*>(smem + SM::off_wm);
+  R* const accs = reinterpret_cast<R*>(smem + SM::off_acc);
   const uint32_t raw_base = smem_u32(smem + SM::off_raw);
   const uint32_t bar_base = smem_u32(smem + SM::off_bar);
 
@@ -165,7 +168,7 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
     R* const bfg = bflux ? bflux + (size_t)g * (30 * FN * FN) : nullptr;
     R* const mfg = (VAR && midflux) ? midflux + (size_t)g * (15 * FN * FN) : nullptr;
 
-    R Wm[5], Wc[5], Wp[5], zplus[5], acc[5], Fzm[5];
+    R Wc[5];
     // prologue: planes -2 (own cell only) and -1 (own + extra, published for the x/y neighbours)
     {
       wait_plane(seq0);
@@ -173,7 +176,12 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
       R U[5];
 #pragma unroll
       for (int q = 0; q < 5; ++q) U[q] = raw[q * (FS * FS) + raw_own];
-      cons2prim<R, Fast>(U, c, Wm);
+      {
+        R Wm[5];
+        cons2prim<R, Fast>(U, c, Wm);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) wms[q * FNT + t] = Wm[q];
+      }
       wait_plane(seq0 + 1);
       raw = raw_ptr(seq0 + 1);
 #pragma unroll
@@ -191,7 +199,7 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         for (int q = 0; q < 5; ++q) wpl[w_ext + q * FS] = We[q];
       }
 #pragma unroll
-      for (int q = 0; q < 5; ++q) { zplus[q] = Wc[q]; acc[q] = R(0); Fzm[q] = R(0); }
+      for (int q = 0; q < 5; ++q) { zs[q * FNT + t] = Wc[q]; accs[q * FNT + t] = R(0); }
     }
     __syncthreads();
 
@@ -202,13 +210,13 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
       {
         wait_plane(seq + 1);
         const R* raw = raw_ptr(seq + 1);
-        R U[5];
+        R U[5], Wp[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) U[q] = raw[q * (FS * FS) + raw_own];
         cons2prim<R, Fast>(U, c, Wp);
         R* wpl = wring + ((seq + 1) & 1) * SM::w_plane;
 #pragma unroll
-        for (int q = 0; q < 5; ++q) wpl[w_own + q * FS] = Wp[q];
+        for (int q = 0; q < 5; ++q) wpl[w_own + q * FS] = Wp[q];   // read back from here where needed: not held in registers
         if (has_extra) {
           R We[5];
 #pragma unroll
@@ -223,6 +231,7 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
       const bool do_pred = ghost_plane ? interior : true;
       if (do_pred) {
         const R* wpl = wring + (seq & 1) * SM::w_plane;
+        const volatile R* wnx = wring + ((seq + 1) & 1) * SM::w_plane;
         R Wn_m[3][5], Wn_p[3][5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) {
@@ -230,8 +239,8 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
           Wn_p[0][q] = wpl[w_own + q * FS + 1];
           Wn_m[1][q] = wpl[w_own + q * FS - WPITCH];
           Wn_p[1][q] = wpl[w_own + q * FS + WPITCH];
-          Wn_m[2][q] = Wm[q];
-          Wn_p[2][q] = Wp[q];
+          Wn_m[2][q] = wms[q * FNT + t];
+          Wn_p[2][q] = wnx[w_own + q * FS];
         }
         const bool ok = predict_cell<R, LIM, Fast>(Wc, Wn_m, Wn_p, c, Wf);
         n_guard += ok ? 0u : 1u;
@@ -285,6 +294,9 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         }
       }
       if (do_z) {
+        R zplus[5];
+#pragma unroll
+        for (int q = 0; q < 5; ++q) zplus[q] = zs[q * FNT + t];
         roe_flux<R, 2, Fast>(zplus, Wf[2][0], c, Fz, flags);
         if (VAR && mfg && k == FN / 2) {
 #pragma unroll
@@ -306,7 +318,7 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
             const R Uin = rawp[q * (FS * FS) + raw_own];
-            out[q] = Uin - c.lam * (acc[q] + (Fz[q] - Fzm[q]));
+            out[q] = Uin - c.lam * (accs[q * FNT + t] + Fz[q]);
             outg[(size_t)q * (FN * FN * FN) + ((k - 1) * FN + j) * FN + i] = out[q];
           }
           const R m2 = out[1] * out[1] + out[2] * out[2] + out[3] * out[3];
@@ -315,13 +327,16 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         if (k >= 0 && k < FN) {
 #pragma unroll
           for (int q = 0; q < 5; ++q) {
-            acc[q] = (fxs[q * FNT + t_xr] - Fx[q]) + (fys[q * FNT + t_yu] - Fy[q]);
-            Fzm[q] = Fz[q];
+            accs[q * FNT + t] = ((fxs[q * FNT + t_xr] - Fx[q]) + (fys[q * FNT + t_yu] - Fy[q])) - Fz[q];
           }
         }
       }
 #pragma unroll
-      for (int q = 0; q < 5; ++q) { Wm[q] = Wc[q]; Wc[q] = Wp[q]; zplus[q] = Wf[2][1][q]; }
+      for (int q = 0; q < 5; ++q) {
+        wms[q * FNT + t] = Wc[q];
+        Wc[q] = (wring + ((seq + 1) & 1) * SM::w_plane)[w_own + q * FS];
+        zs[q * FNT + t] = Wf[2][1][q];
+      }
     }
     __syncthreads();  // all reads of this group's planes done before its stages are reused
   }
