@@ -455,22 +455,26 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
   // ---- R: Roe fluxes at the lower x and the lower y face of the pair -> F[buf]
   auto phaseR = [&](const float* sx, const float* sy, float* fx, float* fy, const St2& Sm1, const St2& Sm2) {
     if (role == 0) {
-      f2 Fx[5], Fy[5];
-      St2 Lx, Ly;
+      // y solve and its stores first, then x: 0.8 % faster than both solves followed by both stores (register lifetimes)
       {
+        f2 Fy[5];
+        St2 Ly;
+        const float* p = sy + iy;
+        Ly.r = lds2(p); Ly.u = lds2(p + 2 * ZNY); Ly.v = lds2(p + 4 * ZNY); Ly.w = lds2(p + 6 * ZNY);
+        Ly.p = lds2(p + 8 * ZNY); Ly.h = lds2(p + 10 * ZNY);
+        roe2<1>(Ly, Sm2, c, Fy);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) sts2(fy + 2 * q * ZNY + iy, Fy[q]);
+      }
+      {
+        f2 Fx[5];
+        St2 Lx;
         const float* p = sx + ix;
         Lx.r = lds2(p); Lx.u = lds2(p + 2 * ZNX); Lx.v = lds2(p + 4 * ZNX); Lx.w = lds2(p + 6 * ZNX);
         Lx.p = lds2(p + 8 * ZNX); Lx.h = lds2(p + 10 * ZNX);
-        p = sy + iy;
-        Ly.r = lds2(p); Ly.u = lds2(p + 2 * ZNY); Ly.v = lds2(p + 4 * ZNY); Ly.w = lds2(p + 6 * ZNY);
-        Ly.p = lds2(p + 8 * ZNY); Ly.h = lds2(p + 10 * ZNY);
-      }
-      roe2<0>(Lx, Sm1, c, Fx);
-      roe2<1>(Ly, Sm2, c, Fy);
+        roe2<0>(Lx, Sm1, c, Fx);
 #pragma unroll
-      for (int q = 0; q < 5; ++q) {
-        sts2(fx + 2 * q * ZNX + ix, Fx[q]);
-        sts2(fy + 2 * q * ZNY + iy, Fy[q]);
+        for (int q = 0; q < 5; ++q) sts2(fx + 2 * q * ZNX + ix, Fx[q]);
       }
     } else if (role == 1) {
       // the face this ghost owns: x = 15.5 (column i = 16: left state SX[16 + 17 j], right state its x- state) or
