@@ -11,10 +11,11 @@ What it established on this pool's B200s (profiles/r2b_issue_microbench.txt):
   * an FFMA2 whose three sources are three DIFFERENT register pairs takes 3 cycles (register-file read bandwidth; 2.2
     when one source repeats from the previous instruction);
   * ALU-pipe instructions (FMNMX, LOP3, IADD3 — 2 pipe cycles each) issued between packed instructions cost 0.5 - 0.8
-    extra cycles each, a scalar FP instruction between packed ones 1.6; MUFU and LDS issue for free beside packed math;
+    extra cycles each, a scalar FP instruction between packed ones 1.6, a MUFU 0.4 (its own pipe takes 8 clocks per warp
+    instruction), an LDS.64 up to 1.0 and an STS.64 more (shared memory moves 128 B per clock and SM);
   * DFMA / DADD take 2 clocks per warp instruction and scheduler (64 FP64 lanes per SM: 37.2 TFLOP/s at 1.965 GHz);
   * so the cost of an instruction stream on one scheduler is, to first order,
-        2 x packed + 1 x (packed with three distinct source pairs) + 1 x scalar FP + ~0.7 x ALU + ~0 x (LDS, MUFU)
+        2 x packed + 1 x (packed with three distinct source pairs) + 1..1.6 x scalar FP + ~0.7 x ALU + ~0.4..1 x (MUFU, LDS)
     cycles, and the FP32 peak of bench.py's roofline (one FFMA per lane per clock) is reached only by a stream of FFMAs.
 
 Usage (GPU box):  python -m harness.issue_microbench [--sass] [--keep DIR]
@@ -57,7 +58,8 @@ def _modes():
     m.append(("2 FADD2 + FADD", lambda i: [f"{A2} x{i}, x{i}, y{i};", f"{A2} z{i}, z{i}, y{i};", f"add.rn.f32 f{i}, f{i}, g{i};"]))
     m.append(("2 FADD2 + 2 IADD3", lambda i: [f"{A2} x{i}, x{i}, y{i};", f"add.s32 p{i}, p{i}, q{i};",
                                               f"{A2} z{i}, z{i}, y{i};", f"add.s32 q{i}, q{i}, p{i};"]))
-    m.append(("4 FADD2 + MUFU.RCP", lambda i: [f"{A2} x{i}, x{i}, y{i};", f"{A2} z{i}, z{i}, y{i};"] * 2 + [f"rcp.approx.ftz.f32 f{i}, f{i};"]))
+    m.append(("4 FADD2 + MUFU.EX2", lambda i: [f"{A2} x{i}, x{i}, y{i};", f"{A2} z{i}, z{i}, y{i};"] * 2 + [f"ex2.approx.ftz.f32 f{i}, f{i};"]))
+    m.append(("MUFU.EX2", lambda i: [f"ex2.approx.ftz.f32 f{i}, f{i};"]))
     m.append(("4 FADD2 + LDS.64 (used)", lambda i: [f"{A2} x{i}, x{i}, y{i};", f"ld.volatile.shared.b64 w{i}, [sa+{4096*i}];",
                                                      f"{A2} z{i}, z{i}, w{i};", f"{A2} x{i}, x{i}, y{i};", f"{A2} z{i}, z{i}, y{i};"]))
     m.append(("4 FADD2 + STS.64", lambda i: [f"st.shared.b64 [sa+{4096*i}], x{i};"] + [f"{A2} x{i}, x{i}, y{i};", f"{A2} z{i}, z{i}, y{i};"] * 2))

@@ -112,3 +112,21 @@ def test_workloads_module_is_arithmetic_free_of_both_sides():
     assert w.n_groups == 8 and w.groups().shape == (8, 5, 20, 20, 20)
     box = wl.assemble_box(w.groups()[:, :, 2:-2, 2:-2, 2:-2], w.shape)
     assert np.array_equal(box, w.U)
+
+
+def test_issue_microbenchmark_generates_and_compiles_for_sm100a(tmp_path):
+    """harness/issue_microbench.py (the evidence behind DESIGN.md section 6's issue-cost model): the generated source
+    compiles for sm_100a and every timed loop still holds the instruction it is named after."""
+    import shutil
+    import subprocess
+    from harness import issue_microbench as mb
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("nvcc not available")
+    cu, exe = tmp_path / "mb.cu", tmp_path / "mb"
+    cu.write_text(mb.generate())
+    subprocess.run([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-o", str(exe), str(cu)], check=True)
+    mix = mb.sass_mix(str(exe))
+    lines = {l[:40].strip(): l[40:] for l in mix.split("\n")}
+    assert "FFMA2" in lines["FFMA2 x*y+z (3 pairs)"] and "FADD2" in lines["FADD2"] and "DFMA" in lines["DFMA (fp64)"]
+    assert "MUFU" in lines["4 FADD2 + MUFU.EX2"] and "LDS" in lines["4 FADD2 + LDS.64 (used)"]
