@@ -14,6 +14,8 @@
 #include <cuda.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 #include "hydro_fused.cuh"  // mbarrier helpers, smem_u32
 
 namespace gh {
@@ -89,55 +91,68 @@ __device__ __forceinline__ void rtvd_line(float* p, int st, const RtvdConst& c) 
 #pragma unroll
     for (int k = 0; k < 4; ++k) A[k][q] = B[k][q] = DA[k][q] = DB[k][q] = 0.0f;
   }
-#pragma unroll 1
-  for (int m0 = 0; m0 < RS + 2; m0 += 4) {
+  // one cell of the march; R = m & 3 (compile time: the queue slots), the three stages switched on at compile time so
+  // that the first cells (which only fill the queues) and the steady part are each straight-line code without merges
+  auto cell = [&](auto r_c, auto u1_c, auto tvd_c, auto store_c, int m) {
+    constexpr int r = decltype(r_c)::value;
+    constexpr bool DO_U1 = decltype(u1_c)::value, DO_TVD = decltype(tvd_c)::value, DO_STORE = decltype(store_c)::value;
+    float uc[5], fr[5], fl[5];
 #pragma unroll
-    for (int r = 0; r < 4; ++r) {
-      const int m = m0 + r;
-      if (m < RS) {
-        float uc[5], fr[5], fl[5];
+    for (int q = 0; q < 5; ++q) uc[q] = p[q * RVOL + m * st];
+    rtvd_split<d>(uc, c, fr, fl);
+    float h[5];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) uc[q] = p[q * RVOL + m * st];
-        rtvd_split<d>(uc, c, fr, fl);
-        float h[5];
+    for (int q = 0; q < 5; ++q) h[q] = frp[q] - fl[q];                 // half-step face flux at m - 1/2
+    if (DO_U1) {
+      // half-step state of cell m-1 and its split fluxes (RT2) -> slot (m - 1) & 3 = (r + 3) & 3
+      float u1[5];
 #pragma unroll
-        for (int q = 0; q < 5; ++q) h[q] = frp[q] - fl[q];                 // half-step face flux at m - 1/2
-        if (m >= 2) {
-          // half-step state of cell m-1 and its split fluxes (RT2) -> slot (m - 1) & 3 = (r + 3) & 3
-          float u1[5];
+      for (int q = 0; q < 5; ++q) u1[q] = fmaf(-c.hlam, h[q] - h_prev[q], up[q]);
+      rtvd_split<d>(u1, c, A[(r + 3) & 3], B[(r + 3) & 3]);
 #pragma unroll
-          for (int q = 0; q < 5; ++q) u1[q] = fmaf(-c.hlam, h[q] - h_prev[q], up[q]);
-          rtvd_split<d>(u1, c, A[(r + 3) & 3], B[(r + 3) & 3]);
+      for (int q = 0; q < 5; ++q) {
+        DA[(r + 3) & 3][q] = A[(r + 3) & 3][q] - A[(r + 2) & 3][q];
+        DB[(r + 3) & 3][q] = B[(r + 3) & 3][q] - B[(r + 2) & 3][q];
+      }
+      if (DO_TVD) {
+        // second-order TVD flux at the face j + 1/2, j = m - 3 (cell n lives in slot n & 3: j in r + 1):
+        // FR = fr_j + vl((fr_j - fr_j-1) / 2, (fr_j+1 - fr_j) / 2), FL = fl_j+1 + vl((fl_j - fl_j+1) / 2, (fl_j+1 - fl_j+2) / 2)
+        // and vl is odd
+        float fu[5];
 #pragma unroll
-          for (int q = 0; q < 5; ++q) {
-            DA[(r + 3) & 3][q] = A[(r + 3) & 3][q] - A[(r + 2) & 3][q];
-            DB[(r + 3) & 3][q] = B[(r + 3) & 3][q] - B[(r + 2) & 3][q];
-          }
-          if (m >= 5) {
-            // second-order TVD flux at the face j + 1/2, j = m - 3 (cell n lives in slot n & 3: j in r + 1):
-            // FR = fr_j + vl((fr_j - fr_j-1) / 2, (fr_j+1 - fr_j) / 2), FL = fl_j+1 + vl((fl_j - fl_j+1) / 2, (fl_j+1 - fl_j+2) / 2)
-            // and vl is odd
-            float fu[5];
+        for (int q = 0; q < 5; ++q) {
+          const float FR = A[(r + 1) & 3][q] + rtvd_vanleer_half(DA[(r + 1) & 3][q], DA[(r + 2) & 3][q]);
+          const float FL = B[(r + 2) & 3][q] - rtvd_vanleer_half(DB[(r + 2) & 3][q], DB[(r + 3) & 3][q]);
+          fu[q] = FR - FL;
+        }
+        if (DO_STORE) {
+          float* o = p + (m - 3) * st;
 #pragma unroll
-            for (int q = 0; q < 5; ++q) {
-              const float FR = A[(r + 1) & 3][q] + rtvd_vanleer_half(DA[(r + 1) & 3][q], DA[(r + 2) & 3][q]);
-              const float FL = B[(r + 2) & 3][q] - rtvd_vanleer_half(DB[(r + 2) & 3][q], DB[(r + 3) & 3][q]);
-              fu[q] = FR - FL;
-            }
-            if (m >= 6) {
-              float* o = p + (m - 3) * st;
-#pragma unroll
-              for (int q = 0; q < 5; ++q) o[q * RVOL] = fmaf(-c.lam, fu[q] - fu_prev[q], o[q * RVOL]);   // RT8
-            }
-#pragma unroll
-            for (int q = 0; q < 5; ++q) fu_prev[q] = fu[q];
-          }
+          for (int q = 0; q < 5; ++q) o[q * RVOL] = fmaf(-c.lam, fu[q] - fu_prev[q], o[q * RVOL]);   // RT8
         }
 #pragma unroll
-        for (int q = 0; q < 5; ++q) { up[q] = uc[q]; h_prev[q] = h[q]; frp[q] = fr[q]; }
+        for (int q = 0; q < 5; ++q) fu_prev[q] = fu[q];
       }
     }
+#pragma unroll
+    for (int q = 0; q < 5; ++q) { up[q] = uc[q]; h_prev[q] = h[q]; frp[q] = fr[q]; }
+  };
+  using Y = std::true_type;
+  using N = std::false_type;
+  using R0 = std::integral_constant<int, 0>;
+  using R1 = std::integral_constant<int, 1>;
+  using R2 = std::integral_constant<int, 2>;
+  using R3 = std::integral_constant<int, 3>;
+  cell(R0{}, N{}, N{}, N{}, 0); cell(R1{}, N{}, N{}, N{}, 1);
+  cell(R2{}, Y{}, N{}, N{}, 2); cell(R3{}, Y{}, N{}, N{}, 3);
+  cell(R0{}, Y{}, N{}, N{}, 4); cell(R1{}, Y{}, Y{}, N{}, 5);
+  cell(R2{}, Y{}, Y{}, Y{}, 6); cell(R3{}, Y{}, Y{}, Y{}, 7);
+#pragma unroll 1
+  for (int m0 = 8; m0 < 20; m0 += 4) {
+    cell(R0{}, Y{}, Y{}, Y{}, m0); cell(R1{}, Y{}, Y{}, Y{}, m0 + 1);
+    cell(R2{}, Y{}, Y{}, Y{}, m0 + 2); cell(R3{}, Y{}, Y{}, Y{}, m0 + 3);
   }
+  cell(R0{}, Y{}, Y{}, Y{}, 20); cell(R1{}, Y{}, Y{}, Y{}, 21);
 }
 
 // all lines of one sweep: `na` x `nb` lines, line (ia, ib) starts at a0 * sa + b0 * sb + ia * sa + ib * sb
