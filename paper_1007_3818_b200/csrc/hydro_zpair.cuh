@@ -192,7 +192,9 @@ __device__ __forceinline__ void zp_run(const CUtensorMap& in_map, float* __restr
 
   // ---- thread -> column (i, j); ghost lanes: rot = the normal is y
   const int t = (int)threadIdx.x, lane = t & 31;
-  const int role = t < 256 ? 0 : 1 + ((t >> 5) & 1);       // warp-uniform: warp 8 upper ghosts, warp 9 lower ghosts
+  // warp-uniform, and read through a shuffle so that the compiler knows it (uniform branches need no reconvergence
+  // bookkeeping): warps 0..7 interior (0), warp 8 upper ghosts (1), warp 9 lower ghosts (2)
+  const int role = __shfl_sync(0xffffffffu, t < 256 ? 0 : 1 + ((t >> 5) & 1), 0);
   int i, j;
   bool rot = false;
   if (role == 0) { j = t >> 4; i = t & 15; }
