@@ -385,10 +385,10 @@ def main():
         # what the step costs the warp schedulers (explanatory, not a roofline): scheduler clocks per cell-update of this
         # run against the issue cost of the kernel's executed instruction mix (profiles/r2b_README.md: packed f32x2 = 2
         # clocks, 3 with three distinct source pairs; measured by harness/issue_microbench.py)
-        clocks = ms_launch * 1e-3 * SM_MAX_GHZ * 1e9 * SM_COUNT * 4 * 32 / cells
-        roofline["issue"] = {"scheduler_clocks_per_cell_update": clocks,
+        sched_clocks = ms_launch * 1e-3 * SM_MAX_GHZ * 1e9 * SM_COUNT * 4 * 32 / cells
+        roofline["issue"] = {"scheduler_clocks_per_cell_update": sched_clocks,
                              "issue_cost_of_instruction_mix": ISSUE_COST_PER_CELL,
-                             "frac_of_issue_bound": ISSUE_COST_PER_CELL / clocks,
+                             "frac_of_issue_bound": ISSUE_COST_PER_CELL / sched_clocks,
                              "clocks_at_target_frac": FLOPS_PER_CELL[0] / (2 * 0.60),
                              "source": "profiles/r2b_README.md, harness/issue_microbench.py"}
 
@@ -521,6 +521,9 @@ def main():
            "guard_cells_per_step": guard_cells / args.steps, "nonpositive_out_per_step": nonpos / args.steps,
            "context_paper": {"gpu_vs_cpu_solver_speedup": 55.0, "overall_speedup_8800GTX": 19.2,
                              "overall_speedup_T10_rtvd": 16.5, "source": "PAPER.md:27,29,13 (other hardware)"}}
+    # the contract's keys keep their types (a local variable once shadowed the clocks record)
+    assert isinstance(out["clocks"], dict) and isinstance(out["roofline"], dict) and isinstance(out["config"], dict)
+    assert isinstance(out["gpu_launches"], int) and out["gpu_launches"] > 0
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
