@@ -98,8 +98,10 @@ __device__ __forceinline__ f2 limited_slope2(f2 a, f2 b) {
     const f2 s = a + b;
     return mk2(mc1(lo(a), lo(b), lo(s)), mc1(hi(a), hi(b), hi(s)));
   } else {
-    const f2 p = a * b, s = a + b;
-    return mk2(vanleer1(lo(a), lo(b), lo(p), lo(s)), vanleer1(hi(a), hi(b), hi(p), hi(s)));
+    // 2 a b / (a + b) with the doubling and the product packed (the same roundings as the scalar form), the
+    // reciprocal and the sign test per lane
+    const f2 p = a * b, q = (p + p) * rcp2(a + b);
+    return mk2(lo(p) > 0.0f ? lo(q) : 0.0f, hi(p) > 0.0f ? hi(q) : 0.0f);
   }
 }
 
