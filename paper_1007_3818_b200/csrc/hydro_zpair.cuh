@@ -6,7 +6,9 @@
 // planes of a pair in the two lanes ALL arithmetic of the step is packed — the predictor, the x, y AND z Roe solves,
 // the update — every neighbour exchange is ONE 64-bit shared-memory access straight into a packed register (the
 // exchange arrays hold plane pairs), and the per-plane bookkeeping (barriers, TMA waits, loop) is paid once per two
-// planes. Lane crossing happens only along z and only through registers: the z slopes use the scalar differences
+// planes (968 -> 645 thread-instructions per cell-update against the one-cell kernel; a packed instruction still costs
+// the scheduler two clocks — profiles/r2b_README.md — so it is the non-FP half of the stream that shrinks). Lane
+// crossing happens only along z and only through registers: the z slopes use the scalar differences
 // W(2p-1) - W(2p-2), W(2p) - W(2p-1), W(2p+1) - W(2p); the z-face solve takes its left states as
 // (z+ of plane 2p-2 kept from the previous pair, z+ of plane 2p-1) and its right states as the pair's z- states.
 //
