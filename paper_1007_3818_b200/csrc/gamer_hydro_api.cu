@@ -597,7 +597,7 @@ int gamer_hydro_step_host(const float* h_in, float* h_out, float* h_bf, int n_gr
   if (rc) return rc;
   const size_t S = (size_t)N + 2 * ghost;
   const size_t in_g = 5 * S * S * S, out_g = (size_t)5 * N * N * N, bf_g = (size_t)30 * N * N;
-  if (chunk_groups <= 0) chunk_groups = 1024;
+  if (chunk_groups <= 0) chunk_groups = 256;   // 101 ms per headline step against 104 ms with 1024 (shorter pipeline tail)
   if (chunk_groups > n_groups) chunk_groups = n_groups;
   {
     std::lock_guard<std::mutex> lk(g_mutex);
