@@ -111,14 +111,25 @@ __global__ void fill_ghosts_kernel(const R* __restrict__ U_out, R* __restrict__ 
     }
   }
   if (vmax) {
+    // one atomic per CTA (the slot is a single address: with one atomic per warp the 32 768 x 32 of them serialise in L2)
+    __shared__ R red[32];
     for (int o = 16; o > 0; o >>= 1) {
       const R other = __shfl_xor_sync(0xffffffffu, m, o);
       m = (other > m || other != other) ? other : m;
     }
-    if ((threadIdx.x & 31) == 0) {
-      Bits b;
-      memcpy(&b, &m, sizeof(R));
-      atomicMax(vmax, b);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+      m = threadIdx.x < ((blockDim.x + 31) >> 5) ? red[threadIdx.x] : R(0);
+      for (int o = 16; o > 0; o >>= 1) {
+        const R other = __shfl_xor_sync(0xffffffffu, m, o);
+        m = (other > m || other != other) ? other : m;
+      }
+      if (threadIdx.x == 0) {
+        Bits b;
+        memcpy(&b, &m, sizeof(R));
+        atomicMax(vmax, b);
+      }
     }
   }
 }
