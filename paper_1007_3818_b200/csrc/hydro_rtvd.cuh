@@ -3,8 +3,10 @@
 // sm_100a: SURVEY.md §8(f) rank 3, the second workload. Readings RT1–RT8 of DESIGN.md §13.
 //
 // One persistent CTA per SM streams 16^3 patch groups. A group with its 3-cell ghost shell is ONE contiguous block
-// of 5 x 22^3 floats = 212 960 B, so it arrives in shared memory by a single 1-D bulk async copy (cp.async.bulk,
-// SASS UBLKCP, completion on an mbarrier) — a tiled tensor map cannot describe it (88-byte rows). The three sweeps
+// of 5 x 22^3 floats = 212 960 B, so it arrives in shared memory by 1-D bulk async copies (cp.async.bulk, SASS
+// UBLKCP, one per variable, completion on one mbarrier) — a tiled tensor map cannot describe it (88-byte rows); the
+// tile is single-buffered (it fills shared memory), so the next group's copy starts variable by variable behind the
+// output copy of the current one, and is prefetched into L2 during the sweeps. The three sweeps
 // run in place in that tile: a thread owns one LINE of 22 cells along the sweep axis and marches along it with the
 // half-step state, the right- / left-moving fluxes of the last four cells and the last face flux in registers; a
 // cell is overwritten three steps after it was last read, so no second tile is needed. Lines are independent: one
@@ -179,21 +181,25 @@ __global__ void __launch_bounds__(RNT, 1)
   }
   __syncthreads();
   uint32_t phase = 0;
+  // one variable of a group's tile: 22^3 floats = 42 592 B (a multiple of 16), its own bulk copy on the common barrier
+  auto load_var = [&](int g, int q) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     tile_s + (uint32_t)(q * RVOL * 4)),
+                 "l"(U_in + (size_t)g * (5 * RVOL) + (size_t)q * RVOL), "r"(RVOL * 4), "r"(bar)
+                 : "memory");
+  };
+  if (threadIdx.x == 0 && (int)blockIdx.x < n_groups) {
+    mbar_expect_tx(bar, RTILE_BYTES);
+    for (int q = 0; q < 5; ++q) load_var((int)blockIdx.x, q);
+  }
   for (int g = (int)blockIdx.x; g < n_groups; g += (int)gridDim.x) {
-    if (threadIdx.x == 0) {
-      // the tile's previous contents were read through the generic proxy: order those reads before the async write
-      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-      mbar_expect_tx(bar, RTILE_BYTES);
-      asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(tile_s),
-                   "l"(U_in + (size_t)g * (5 * RVOL)), "r"(RTILE_BYTES), "r"(bar)
-                   : "memory");
-    }
     mbar_wait(bar, phase);
     phase ^= 1u;
-    // the tile is single-buffered (213 KB), so the next group's copy cannot overlap the sweeps; pull it into L2 meanwhile
-    if (threadIdx.x == 0 && g + (int)gridDim.x < n_groups)
-      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(U_in + (size_t)(g + (int)gridDim.x) * (5 * RVOL)),
-                   "r"(RTILE_BYTES)
+    const int g_next = g + (int)gridDim.x;
+    // the tile is single-buffered (213 KB): the next group's copy starts variable by variable behind the output copy
+    // below; pull it into L2 meanwhile
+    if (threadIdx.x == 0 && g_next < n_groups)
+      asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(U_in + (size_t)g_next * (5 * RVOL)), "r"(RTILE_BYTES)
                    : "memory");
     // x fastest: cell (x, y, z) of variable q at q RVOL + z 484 + y 22 + x (RT7)
     if (SWEEP == 0) {
@@ -211,11 +217,19 @@ __global__ void __launch_bounds__(RNT, 1)
     }
     __syncthreads();
     float* const og = U_out + (size_t)g * (5 * RN * RN * RN);
-    for (int e = (int)threadIdx.x; e < 5 * RN * RN * RN; e += RNT) {
-      const int x = e & 15, y = (e >> 4) & 15, z = (e >> 8) & 15, q = e >> 12;
-      og[e] = tile[q * RVOL + ((z + RG) * RS + (y + RG)) * RS + (x + RG)];
+    if (threadIdx.x == 0 && g_next < n_groups) mbar_expect_tx(bar, RTILE_BYTES);
+    for (int q = 0; q < 5; ++q) {
+      for (int e = (int)threadIdx.x; e < RN * RN * RN; e += RNT) {
+        const int x = e & 15, y = (e >> 4) & 15, z = e >> 8;
+        og[q * (RN * RN * RN) + e] = tile[q * RVOL + ((z + RG) * RS + (y + RG)) * RS + (x + RG)];
+      }
+      __syncthreads();   // every read of variable q's part of the tile is done: the next group's variable q may land
+      if (threadIdx.x == 0 && g_next < n_groups) {
+        // those reads went through the generic proxy: order them before the async write
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+        load_var(g_next, q);
+      }
     }
-    __syncthreads();   // every read of the tile is done before the next group's copy lands
   }
 }
 
