@@ -374,7 +374,10 @@ int max_speed_impl(const R* U, int n_groups, int N, int ghost, double gamma, dou
   const int threads = 256;
   long long want = (n_cells + threads - 1) / threads;
   const int grid = (int)(want < (long long)g_state.sm_count * 16 ? want : (long long)g_state.sm_count * 16);
-  gh::max_speed_kernel<R, Bits><<<grid, threads, 0, stream>>>(U, n_cells, N, ghost, (R)gamma, slot);
+  if (N == 16 && ghost == 2)
+    gh::max_speed_kernel<R, Bits, 16, 2><<<grid, threads, 0, stream>>>(U, n_cells, N, ghost, (R)gamma, slot);
+  else
+    gh::max_speed_kernel<R, Bits, 0, 0><<<grid, threads, 0, stream>>>(U, n_cells, N, ghost, (R)gamma, slot);
   g_launches.fetch_add(1);
   CK(cudaGetLastError());
   Bits bits = 0;

@@ -11,8 +11,10 @@ namespace gh {
 // S = N + 2 ghost (ghost = 0 for U_out). The result is accumulated with an integer atomicMax on the bit pattern
 // (non-negative IEEE values order like unsigned integers; a NaN orders above them all, so a state holding NaN gives
 // a NaN maximum and the caller's dt check trips), so *out must be zeroed before the launch.
-template <class R, class Bits>
-__global__ void max_speed_kernel(const R* __restrict__ U, long long n_cells, int N, int ghost, R gamma, Bits* out) {
+// NC, GC > 0: compile-time patch size and ghost width (the 16 / 2 of the configs: the index arithmetic becomes shifts).
+template <class R, class Bits, int NC, int GC>
+__global__ void max_speed_kernel(const R* __restrict__ U, long long n_cells, int N_rt, int ghost_rt, R gamma, Bits* out) {
+  const int N = NC > 0 ? NC : N_rt, ghost = NC > 0 ? GC : ghost_rt;
   const int S = N + 2 * ghost;
   const long long S3 = (long long)S * S * S, N3 = (long long)N * N * N;
   R m = R(0);
