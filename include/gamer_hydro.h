@@ -49,7 +49,8 @@ enum {
                                   unknown limiter, misaligned pointer */
   GAMER_HYDRO_UNSUPPORTED = 2, /* shape the library has no kernel for */
   GAMER_HYDRO_CUDA_ERROR = 3,  /* a CUDA call failed; gamer_hydro_strerror(3) carries the CUDA message */
-  GAMER_HYDRO_NOT_SM100 = 4    /* the device is not compute capability 10.x */
+  GAMER_HYDRO_NOT_SM100 = 4,   /* the device is not compute capability 10.x */
+  GAMER_HYDRO_TOO_LARGE = 5    /* gamer_hydro_max_speed_noalloc: more patch groups than its fixed scratch array holds */
 };
 
 enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1, GAMER_HYDRO_MC = 2 /* monotonized central, R3b */ };
@@ -127,6 +128,39 @@ int gamer_hydro_step_host(const float* h_U_in_with_ghosts, float* h_U_out, float
  * S = N + 2 ghost (ghost = 0 for a U_out array). Synchronises `stream`. */
 int gamer_hydro_max_speed(const void* U, int bytes_per_real, int n_groups, int N, int ghost, double gamma,
                           double* h_max, cudaStream_t stream);
+
+/* The CFL signal speed of gamer_hydro_max_speed (reading R15, fp32) for callers that cannot afford a device
+ * allocation, now or later in the run. Two kinds of caller are meant. An AMR code that fills the GPU with its patch
+ * pools at start-up: a cudaMalloc made on its behalf in the middle of a run can fail for lack of memory, hours in. And
+ * a time loop that keeps copies and kernels of several streams in flight ("concurrent execution between CPU
+ * and GPU"): cudaMalloc and cudaFree wait for the whole device, so one allocation stalls every stream. The other
+ * entry points allocate on first use (gamer_hydro_alloc: status block, scratch, staging buffers). This one calls no
+ * cudaMalloc, no cudaFree and no library routine that allocates, and does not run gamer_hydro_alloc: its only working
+ * memory is one fixed array inside the library image, 256.25 KiB (a 256-byte header and one word per patch group),
+ * which every GPU that loads the library holds until the process exits.
+ *   U       float[n_groups][5][S][S][S], S = N + 2*ghost (ghost = 0 for a U_out array), DEVICE, read-only
+ *   d_max   one float, DEVICE, 4-byte aligned, owned by the caller: receives the maximum over the interior cells of all
+ *           groups of |vx| + |vy| + |vz| + 3 c_s; NaN if any cell is NaN (same rule and same arithmetic as
+ *           gamer_hydro_max_speed, which returns the value to the host instead)
+ * Enqueues a 4-byte clear of the array's counter and one kernel on `stream` and returns without synchronising; read
+ * *d_max on the same stream (for instance with cudaMemcpyAsync into pinned memory) when it is needed.
+ * Limits and rules:
+ *   - 1 <= n_groups <= gamer_hydro_max_speed_noalloc_limit() (65536); more returns GAMER_HYDRO_TOO_LARGE and enqueues
+ *     nothing. Split a larger batch and take the maximum of the parts.
+ *   - Call it with the device that owns U, d_max and `stream` current. The first call on each device looks up where that
+ *     device keeps its copy of the array (cudaGetSymbolAddress) and checks the compute capability; make that first call
+ *     before any stream capture begins. Later calls only enqueue.
+ *   - All calls on one device share the array, and it keeps the last call's contents. The counter that must start at
+ *     zero is cleared by every call itself. Two calls whose kernels can overlap on the GPU (different streams with no
+ *     event between them) race on the array and both results are then undefined: order them with an event, or keep
+ *     them on one stream, where they run one after the other.
+ * Errors: GAMER_HYDRO_INVALID_ARG (null or misaligned pointer, n_groups < 1, N < 1, ghost < 0, gamma <= 1),
+ * GAMER_HYDRO_TOO_LARGE, GAMER_HYDRO_NOT_SM100, GAMER_HYDRO_UNSUPPORTED (device ordinal >= 64), GAMER_HYDRO_CUDA_ERROR. */
+int gamer_hydro_max_speed_noalloc(const float* U, int n_groups, int N, int ghost, float gamma, float* d_max,
+                                  cudaStream_t stream);
+
+/* Largest n_groups gamer_hydro_max_speed_noalloc accepts (65536: twice the headline batch of 32768 groups). */
+int gamer_hydro_max_speed_noalloc_limit(void);
 
 /* Same-level ghost-shell refill (reading R16): rebuilds every stored cell of U_in_with_ghosts
  * [G][5][S][S][S] — interior and ghost shell — from the interior arrays U_out [G][5][N][N][N] of the groups that

@@ -21,7 +21,8 @@ PATH_AUTO, PATH_GENERIC, PATH_FUSED, PATH_FUSED_SCALAR, PATH_FUSED_DUO = 0, 1, 2
 EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_hydro_step_f64",
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
            "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance",
-           "gamer_hydro_step_grid", "gamer_hydro_set_guard_map", "gamer_rtvd_step", "gamer_hydro_step_ex", "gamer_hydro_step_ex_f64"]
+           "gamer_hydro_step_grid", "gamer_hydro_set_guard_map", "gamer_rtvd_step", "gamer_hydro_step_ex", "gamer_hydro_step_ex_f64",
+           "gamer_hydro_max_speed_noalloc", "gamer_hydro_max_speed_noalloc_limit"]
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
@@ -46,6 +47,8 @@ def lib():
         L.gamer_hydro_status.argtypes = [C.POINTER(C.c_ulonglong), C.POINTER(C.c_ulonglong)]
         L.gamer_hydro_set_path.argtypes = [i]
         L.gamer_hydro_max_speed.argtypes = [vp, i, i, i, i, d, C.POINTER(C.c_double), vp]
+        L.gamer_hydro_max_speed_noalloc.argtypes = [vp, i, i, i, f, vp, vp]
+        L.gamer_hydro_max_speed_noalloc_limit.argtypes = []
         L.gamer_hydro_fill_ghosts.argtypes = [vp, vp, i, i, i, i, i, i, i, i, i, vp]
         L.gamer_hydro_step_grid.argtypes = [vp, vp, vp, vp, i, i, i, i, i, f, f, f, i, vp]
         L.gamer_hydro_advance.argtypes = [vp, vp, vp, i, i, i, i, i, i, i, i, i, f, f, f, i, vp, vp]
@@ -150,6 +153,31 @@ def gamer_hydro_max_speed(U, N=16, ghost=2, gamma=5.0 / 3.0, stream=None):
     _check(lib().gamer_hydro_max_speed(U.data_ptr(), _real_bytes(U), U.shape[0], N, ghost, gamma, C.byref(out),
                                        _stream_ptr(stream)))
     return float(out.value)
+
+
+def gamer_hydro_max_speed_noalloc_limit():
+    """Largest number of patch groups gamer_hydro_max_speed_noalloc takes in one call."""
+    return int(lib().gamer_hydro_max_speed_noalloc_limit())
+
+
+def gamer_hydro_max_speed_noalloc(U, d_max, N=16, ghost=2, gamma=5.0 / 3.0, stream=None):
+    """Signal-speed maximum (R15) of a float32 device array [G][5][S][S][S] into d_max, a float32 CUDA tensor with one
+    element that the caller owns. For callers that must not trigger a device allocation (an AMR code that has filled the
+    GPU with its own pools; a multi-stream time loop that a device-wide cudaMalloc would stall): the library keeps the
+    partial maxima in a fixed array of its own, at most gamer_hydro_max_speed_noalloc_limit() groups per call. Nothing
+    is allocated here either: pass d_max in, read it back on the same stream. Enqueues and returns d_max; calls that
+    could overlap on the GPU must be ordered by the caller (they share that array). Make the first call on a device
+    outside any stream capture."""
+    S = N + 2 * ghost
+    if U.dim() != 5 or tuple(U.shape[1:]) != (5, S, S, S):
+        raise GamerHydroError("U must be [n_groups][5][%d][%d][%d]" % (S, S, S))
+    if not (U.is_cuda and U.dtype == torch.float32 and U.is_contiguous()):
+        raise GamerHydroError("U must be a contiguous CUDA float32 tensor")
+    if not (d_max.is_cuda and d_max.dtype == torch.float32 and d_max.numel() == 1 and d_max.device == U.device):
+        raise GamerHydroError("d_max must be a one-element CUDA float32 tensor on the device of U")
+    _check(lib().gamer_hydro_max_speed_noalloc(U.data_ptr(), U.shape[0], N, ghost, gamma, d_max.data_ptr(),
+                                               _stream_ptr(stream)))
+    return d_max
 
 
 def gamer_hydro_fill_ghosts(U_out, U_in_with_ghosts, grid, N=16, ghost=2, bc=(BC_PERIODIC,) * 3, stream=None):

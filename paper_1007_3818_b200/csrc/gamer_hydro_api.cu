@@ -682,6 +682,128 @@ int gamer_hydro_set_guard_map(unsigned char* device_map) {
   return 0;
 }
 
+}  // extern "C" (re-opened below, after the no-allocation section)
+
+// ---------------------------------------------------------------------------------------------------------------
+// gamer_hydro_max_speed_noalloc: the CFL signal-speed maximum (R15) for callers that must not trigger a device
+// allocation. Who that is: an AMR code that sized its patch pools to fill the GPU at start-up (a cudaMalloc issued by
+// this library in the middle of a run can then fail for lack of memory, long after the run began), and a time loop
+// that keeps copies and kernels of several streams in flight (cudaMalloc and cudaFree wait for the whole device, so an
+// allocation inside the loop stalls every one of those streams). gamer_hydro_max_speed goes through the library's
+// set-up, which allocates the status block its reduction slot lives in; this variant keeps its partial maxima in the
+// fixed array below instead and writes the result to a device address the caller supplies.
+//
+// The array is part of the loaded library image: every GPU that loads libgamer_hydro.so holds these 256.25 KiB until
+// the process exits, whether or not this entry point is ever called. All calls on a device share it and it keeps
+// whatever the last call left in it.
+constexpr int kNoAllocMaxGroups = 65536;   // twice the headline batch of BASELINE.json:configs[3]
+constexpr int kNoAllocHeader = 64;         // words: [0] = number of CTAs that have published their maximum
+constexpr int kNoAllocMaxDevices = 64;
+static __device__ __align__(256) unsigned int g_noalloc_scratch[kNoAllocHeader + kNoAllocMaxGroups];
+
+namespace {
+
+// One CTA per patch group: maximum of |vx| + |vy| + |vz| + 3 c_s over the group's interior cells (the arithmetic of
+// gh::max_speed_kernel, same NaN rule: a NaN cell makes the maximum NaN) -> scratch[header + group]. The CTA that
+// publishes last (ticket in scratch[0], which must be 0 when the kernel starts) reduces the per-group maxima and
+// writes *d_max. `scratch` is the DEVICE address of g_noalloc_scratch, looked up by the host (see below).
+template <int NC, int GC>
+__global__ void max_speed_noalloc_kernel(const float* __restrict__ U, int N_rt, int ghost_rt, float gamma,
+                                         unsigned int* scratch, float* __restrict__ d_max) {
+  const int N = NC > 0 ? NC : N_rt, ghost = NC > 0 ? GC : ghost_rt;
+  const int S = N + 2 * ghost;
+  const long long S3 = (long long)S * S * S;
+  const float* Ug = U + (long long)blockIdx.x * 5 * S3;
+  __shared__ float red[32];
+  __shared__ bool last;
+  auto nanmax = [](float a, float b) { return (b > a || b != b) ? b : a; };
+  auto block_max = [&](float m) -> float {   // valid in thread 0
+    for (int o = 16; o > 0; o >>= 1) m = nanmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = m;
+    __syncthreads();
+    if (threadIdx.x < 32) {
+      m = threadIdx.x < ((blockDim.x + 31) >> 5) ? red[threadIdx.x] : 0.0f;
+      for (int o = 16; o > 0; o >>= 1) m = nanmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    }
+    __syncthreads();
+    return m;
+  };
+  float m = 0.0f;
+  for (int r = threadIdx.x; r < N * N * N; r += blockDim.x) {
+    const int i = r % N, j = (r / N) % N, k = r / (N * N);
+    const float* p = Ug + ((long long)(k + ghost) * S + (j + ghost)) * S + (i + ghost);
+    const float rho = p[0], mx = p[S3], my = p[2 * S3], mz = p[3 * S3], E = p[4 * S3];
+    const float ir = 1.0f / rho;
+    float P = (gamma - 1.0f) * (E - 0.5f * (mx * mx + my * my + mz * mz) * ir);
+    P = P > 0.0f ? P : 0.0f;
+    const float v = (fabsf(mx) + fabsf(my) + fabsf(mz)) * ir + 3.0f * sqrtf(gamma * P * ir);
+    m = nanmax(m, v);
+  }
+  m = block_max(m);
+  if (threadIdx.x == 0) {
+    scratch[kNoAllocHeader + blockIdx.x] = __float_as_uint(m);
+    __threadfence();                                        // the maximum is visible before the ticket is
+    last = atomicAdd(scratch, 1u) == gridDim.x - 1;
+  }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  const volatile unsigned int* part = scratch + kNoAllocHeader;   // written by other CTAs: read past L1
+  m = 0.0f;
+  for (int g = threadIdx.x; g < (int)gridDim.x; g += blockDim.x) m = nanmax(m, __uint_as_float(part[g]));
+  m = block_max(m);
+  if (threadIdx.x == 0) *d_max = m;
+}
+
+std::mutex g_noalloc_mutex;
+unsigned int* g_noalloc_addr[kNoAllocMaxDevices] = {};   // per device: DEVICE address of g_noalloc_scratch, 0 = not set up
+
+// In host code the name g_noalloc_scratch is only a handle for the symbol, not an address the GPU can use, and every
+// device that loads the library has its own copy of the array at its own address. Hence: once per device, with that
+// device current, ask the runtime where the copy lives, and hand that pointer to the kernel.
+int noalloc_scratch_of_current_device(unsigned int** out) {
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return GAMER_HYDRO_UNSUPPORTED;
+  std::lock_guard<std::mutex> lk(g_noalloc_mutex);
+  if (!g_noalloc_addr[dev]) {
+    int major = 0;
+    CK(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    if (major != 10) return GAMER_HYDRO_NOT_SM100;
+    void* p = nullptr;
+    CK(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p) return GAMER_HYDRO_CUDA_ERROR;
+    g_noalloc_addr[dev] = static_cast<unsigned int*>(p);
+  }
+  *out = g_noalloc_addr[dev];
+  return 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+int gamer_hydro_max_speed_noalloc_limit(void) { return kNoAllocMaxGroups; }
+
+int gamer_hydro_max_speed_noalloc(const float* U, int n_groups, int N, int ghost, float gamma, float* d_max,
+                                  cudaStream_t stream) {
+  if (!U || !d_max || n_groups < 1 || N < 1 || ghost < 0 || !(gamma > 1.0f) || ((uintptr_t)d_max & 3))
+    return GAMER_HYDRO_INVALID_ARG;
+  if (n_groups > kNoAllocMaxGroups) return GAMER_HYDRO_TOO_LARGE;   // the fixed array has one word per group
+  unsigned int* scratch = nullptr;
+  int rc = noalloc_scratch_of_current_device(&scratch);
+  if (rc) return rc;
+  // the ticket must start at zero, whatever the previous call (or a call that died half-way) left behind
+  CK(cudaMemsetAsync(scratch, 0, sizeof(unsigned int), stream));
+  if (N == 16 && ghost == 2)
+    max_speed_noalloc_kernel<16, 2><<<n_groups, 256, 0, stream>>>(U, N, ghost, gamma, scratch, d_max);
+  else
+    max_speed_noalloc_kernel<0, 0><<<n_groups, 256, 0, stream>>>(U, N, ghost, gamma, scratch, d_max);
+  g_launches.fetch_add(1);
+  CK(cudaGetLastError());
+  return 0;
+}
+
 unsigned long long gamer_hydro_launch_count(void) { return g_launches.load(); }
 
 const char* gamer_hydro_strerror(int code) {
@@ -691,6 +813,9 @@ const char* gamer_hydro_strerror(int code) {
     case GAMER_HYDRO_UNSUPPORTED: return "unsupported shape for the requested kernel path";
     case GAMER_HYDRO_CUDA_ERROR: return g_state.cuda_msg;
     case GAMER_HYDRO_NOT_SM100: return "device is not compute capability 10.x (sm_100a required)";
+    case GAMER_HYDRO_TOO_LARGE:
+      return "batch exceeds the fixed scratch array of gamer_hydro_max_speed_noalloc (65536 patch groups at most): "
+             "split the batch or call gamer_hydro_max_speed";
     default: return "unknown error code";
   }
 }
