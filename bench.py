@@ -200,7 +200,8 @@ def main():
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--cpu-groups", type=int, default=4096,
                     help="groups in the oracle sample (cpu_baseline): 16.8 M cell-updates, about 15 core-seconds")
-    ap.add_argument("--ref-groups", type=int, default=2048, help="groups per step of the --impl reference arm")
+    ap.add_argument("--ref-groups", type=int, default=512,
+                    help="groups per step of the --impl reference arm (its 128^3 box holds 512)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-multistep", action="store_true")

@@ -44,7 +44,7 @@ __global__ void max_speed_kernel(const R* __restrict__ U, long long n_cells, int
 // Ghost-shell refill on one uniform grid of gx x gy x gz groups (group index x-fastest): every stored cell of
 // U_in — interior and ghost — is gathered from the interior arrays U_out of the group that owns it, with periodic
 // wrap (bc = 0) or outflow = nearest interior cell (bc = 1) per axis (R16). Pure data movement; one CTA per
-// (group, z plane), 32-bit index arithmetic. Since every cell passes through a thread with all five variables, the
+// group, 32-bit index arithmetic. Since every cell passes through a thread with all five variables, the
 // kernel also accumulates the signal-speed maximum of the NEW state (ghost cells are copies of interior cells, so
 // they do not change it): vmax may be null.
 template <class R> struct alignas(2 * sizeof(R)) Vec2 { R a, b; };

@@ -4,8 +4,8 @@
 //   lanes (x, y)  for the '+' face states, the '-' face states, their own-direction fluxes and the x / y Roe solves
 //                 (the y lane holds its velocity components as (v, u, w) so that slot 1 is the normal one),
 //   lanes (z-, z+) for the two z face states and their fluxes (same slot orders, slot 3 = w is normal in both).
-// The packed forms keep the issue-slot saving of hydro_pair.cuh (half the slots per FLOP) without its register
-// appetite, so five warps per scheduler stay resident to hide the dependent-issue latency (profiles/r1c_README.md).
+// The packed forms (helpers in hydro_f2.cuh, shared with hydro_zpair.cuh) keep the issue-slot saving of packed math
+// (half the slots per FLOP) without the register appetite of round 1's two-cells-per-thread kernel (since removed), so five warps per scheduler stay resident to hide the dependent-issue latency (profiles/r1c_README.md).
 // Schedule per plane: TWO split (arrive / wait) mbarrier barriers — "states of plane k published" and "x / y fluxes of
 // plane k published" — instead of __syncthreads; everything a neighbour publishes is double-buffered and consumed one
 // phase later, and the work between an arrive and its wait absorbs the skew between warps.

@@ -1,6 +1,6 @@
 """GPU tests (-m gpu) of the steps either side of the hot path: the CFL signal-speed
 maximum (R15), the same-level ghost-shell refill (R16) and the device-resident multi-step driver. References: the
-numpy harness of paper_1007_3818_b200/workloads.py (pure data movement / the R15 formula in fp64) and, for the
+numpy harness of harness/workloads.py (pure data movement / the R15 formula in fp64) and, for the
 multi-step run, the fp64 oracle stepped with the time steps the device reports."""
 import numpy as np
 import pytest
