@@ -13,9 +13,11 @@
  * Concurrency: the library serves ONE device per process (the first one it is used on; a second device returns
  * GAMER_HYDRO_INVALID_ARG: run one process per GPU). gamer_hydro_step / _f64, gamer_hydro_max_speed,
  * gamer_hydro_fill_ghosts, gamer_hydro_step_grid and gamer_hydro_advance may be called concurrently from several
- * host threads on different streams: every call that reduces on the device takes its own reduction slot (64 in
- * flight), and calls that need the library's one scratch buffer (the shape-generic kernels) are chained by an event,
- * i.e. they run one after the other. Process-global and NOT thread-safe: gamer_hydro_set_path,
+ * host threads on different streams: gamer_hydro_max_speed and gamer_hydro_advance LEASE a reduction slot of their own
+ * for as long as they run (an advance: for all its steps) — 64 leases at a time, the 65th concurrent call returns
+ * GAMER_HYDRO_BUSY rather than share one — and calls that need the library's one scratch buffer (the shape-generic
+ * kernels) are chained by an event, i.e. they run one after the other; growing that buffer, reading its address and
+ * enqueueing on it happen under one lock. Process-global and NOT thread-safe: gamer_hydro_set_path,
  * gamer_hydro_set_guard_map, gamer_hydro_status (test / diagnostic plumbing), gamer_hydro_step_host (it owns the
  * library's three internal streams) and gamer_hydro_advance on the DUO path (it ping-pongs with one library-owned
  * array).
@@ -50,7 +52,8 @@ enum {
   GAMER_HYDRO_UNSUPPORTED = 2, /* shape the library has no kernel for */
   GAMER_HYDRO_CUDA_ERROR = 3,  /* a CUDA call failed; gamer_hydro_strerror(3) carries the CUDA message */
   GAMER_HYDRO_NOT_SM100 = 4,   /* the device is not compute capability 10.x */
-  GAMER_HYDRO_TOO_LARGE = 5    /* gamer_hydro_max_speed_noalloc: more patch groups than its fixed scratch array holds */
+  GAMER_HYDRO_TOO_LARGE = 5,   /* gamer_hydro_max_speed_noalloc: more patch groups than its fixed scratch array holds */
+  GAMER_HYDRO_BUSY = 6         /* gamer_hydro_max_speed / gamer_hydro_advance: 64 such calls are already in flight */
 };
 
 enum { GAMER_HYDRO_MINMOD = 0, GAMER_HYDRO_VANLEER = 1, GAMER_HYDRO_MC = 2 /* monotonized central, R3b */ };
@@ -186,9 +189,13 @@ int gamer_hydro_step_grid(const float* U_with_ghosts, float* U_out, float* bound
  * the last step; h_dts (HOST, n_steps floats, may be NULL) receives the time steps taken. One 4-byte
  * device-to-host read and one stream synchronisation per step. With GAMER_HYDRO_PATH_FUSED_DUO selected, a fully
  * periodic grid of 16^3 groups uses gamer_hydro_step_grid instead of step + refill, ping-ponging between U and a
- * second ghosted array the library allocates (and keeps). A state without a finite positive signal speed (a NaN or
- * non-positive cell makes the device maximum NaN) ends the loop with GAMER_HYDRO_INVALID_ARG; on every return,
- * error or not, U holds the state after the steps completed so far. */
+ * second ghosted array the library allocates (and keeps). A state without a finite positive signal speed ends the
+ * loop with GAMER_HYDRO_INVALID_ARG: a NaN cell makes the device maximum NaN, and so does a cell with rho <= 0 as long as
+ * its pressure expression stays positive (the sound speed is then the root of a negative number). NOT caught: a cell with
+ * rho > 0 and P <= 0 enters with c_s = 0 (R15's max(P, 0)), and a cell with rho < 0 whose clamped pressure is 0 drops out
+ * of the maximum; the loop then continues on that state with the time step of the other cells — such cells are counted,
+ * never repaired (gamer_hydro_status, R10). On every return, error or not, U holds the state after the steps completed
+ * so far. */
 int gamer_hydro_advance(float* U_with_ghosts, float* U_out, float* boundary_fluxes, int gx, int gy, int gz, int N,
                         int ghost, int bc_x, int bc_y, int bc_z, int n_steps, float cfl, float dx, float gamma,
                         int limiter, float* h_dts, cudaStream_t stream);
@@ -216,7 +223,9 @@ int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonp
  * the parity maximum). With device_map != NULL every later step call marks the cells whose predicted states fell
  * back to first order: device_map[g][k+1][j+1][i+1] = 1, unsigned char [n_groups][N+2][N+2][N+2] in DEVICE memory,
  * owned and zeroed by the caller, indices -1 .. N per axis (first ghost layer included). NULL (the default) switches
- * it off. Process-global, synchronises the device; the map is written on the rare fallback path only. */
+ * it off. Process-global, synchronises the device; the map is written on the rare fallback path only. The group index
+ * g is the one of the step call's own batch: do not combine the map with gamer_hydro_step_host, which steps the batch
+ * in chunks (every chunk would mark the map from g = 0 again). */
 int gamer_hydro_set_guard_map(unsigned char* device_map);
 
 /* Forces a kernel path (tests, benchmarking); GAMER_HYDRO_PATH_AUTO restores the default. */

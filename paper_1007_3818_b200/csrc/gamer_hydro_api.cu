@@ -52,13 +52,32 @@ struct State {
 State g_state;
 std::mutex g_mutex;
 std::atomic<unsigned long long> g_launches{0};
-std::atomic<unsigned int> g_slot{0};
 
-constexpr int kReduceSlots = 64;    // signal-speed maxima of concurrent max_speed / step_grid / advance calls
+constexpr int kReduceSlots = 64;    // signal-speed maxima of concurrent max_speed / advance calls
+unsigned long long g_slot_busy = 0; // bit s set: slot s is leased (under g_mutex)
 
-// every call that reduces a signal-speed maximum on the device takes its own 8-byte slot (round robin), so calls on
-// different streams do not share one
-unsigned long long* next_reduce_slot() { return g_state.status + 2 + (g_slot.fetch_add(1) % kReduceSlots); }
+// Every call that reduces a signal-speed maximum on the device and READS it back leases its own 8-byte slot for as
+// long as it runs (gamer_hydro_advance: for all its steps), so calls on other threads and streams can neither zero
+// it nor add their maxima to it. With all 64 leased the call fails with GAMER_HYDRO_BUSY instead of sharing a slot.
+// Slot kReduceSlots is a sink nobody reads (the public gamer_hydro_step_grid, which returns before its kernel ran).
+struct SlotLease {
+  int idx = -1;
+  SlotLease() {
+    std::lock_guard<std::mutex> lk(g_mutex);
+    for (int s = 0; s < kReduceSlots; ++s)
+      if (!(g_slot_busy >> s & 1ull)) { g_slot_busy |= 1ull << s; idx = s; break; }
+  }
+  ~SlotLease() {
+    if (idx < 0) return;
+    std::lock_guard<std::mutex> lk(g_mutex);
+    g_slot_busy &= ~(1ull << idx);
+  }
+  SlotLease(const SlotLease&) = delete;
+  SlotLease& operator=(const SlotLease&) = delete;
+  bool ok() const { return idx >= 0; }
+  unsigned long long* ptr() const { return g_state.status + 2 + idx; }
+};
+unsigned long long* sink_reduce_slot() { return g_state.status + 2 + kReduceSlots; }
 
 constexpr int kGenericChunk = 512;  // groups per generic-path launch (bounds the scratch buffer)
 
@@ -93,9 +112,9 @@ int init_locked(int device) {
   CK(cudaSetDevice(device));
   g_state.sm_count = prop.multiProcessorCount;
   g_state.smem_per_sm = (int)prop.sharedMemPerMultiprocessor;
-  // [0] guard cells, [1] non-positive outputs, [2] bit pattern of the running signal-speed maximum
-  CK(cudaMalloc(&g_state.status, (2 + kReduceSlots) * sizeof(unsigned long long)));
-  CK(cudaMemset(g_state.status, 0, (2 + kReduceSlots) * sizeof(unsigned long long)));
+  // [0] guard cells, [1] non-positive outputs, [2 ..] leased reduction slots, then one sink slot
+  CK(cudaMalloc(&g_state.status, (2 + kReduceSlots + 1) * sizeof(unsigned long long)));
+  CK(cudaMemset(g_state.status, 0, (2 + kReduceSlots + 1) * sizeof(unsigned long long)));
   CK(cudaEventCreateWithFlags(&g_state.scratch_free, cudaEventDisableTiming));
   int rc;
   if ((rc = set_fused_attr<float, 0, true>())) return rc;
@@ -137,8 +156,9 @@ int ensure_init() {
   return init_locked(dev);
 }
 
-int ensure_scratch(size_t bytes) {
-  std::lock_guard<std::mutex> lk(g_mutex);
+// grows the generic-path scratch; g_mutex must be HELD (a grow frees the old buffer: nobody may read the pointer or
+// enqueue work on it meanwhile)
+int ensure_scratch_locked(size_t bytes) {
   if (g_state.scratch_bytes >= bytes) return 0;
   if (g_state.scratch) {
     CK(cudaDeviceSynchronize());
@@ -149,6 +169,11 @@ int ensure_scratch(size_t bytes) {
   CK(cudaMalloc(&g_state.scratch, bytes));
   g_state.scratch_bytes = bytes;
   return 0;
+}
+
+int ensure_scratch(size_t bytes) {
+  std::lock_guard<std::mutex> lk(g_mutex);
+  return ensure_scratch_locked(bytes);
 }
 
 template <class R>
@@ -285,16 +310,18 @@ template <class R>
 int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int ghost, R dt, R dx, R gamma,
                    int limiter, cudaStream_t stream, int flags = 0, R* midflux = nullptr) {
   const int chunk = n_groups < kGenericChunk ? n_groups : kGenericChunk;
-  int rc = ensure_scratch(generic_scratch_bytes<R>(chunk, N, ghost));
-  if (rc) return rc;
   const gh::GenericShape sh = gh::make_shape(N, ghost);
   const gh::GasConst<R> c = gh::make_consts<R>(dt, dx, gamma);
-  R* FS = reinterpret_cast<R*>(g_state.scratch);
-  R* FL = FS + (size_t)chunk * sh.fs_stride;
   const long long ne = (long long)sh.E * sh.E * sh.E, nf = 3LL * (N + 1) * N * N, nc = (long long)N * N * N;
   // ONE scratch buffer serves every stream: calls on different streams are chained by an event (the predictor of the
-  // next call waits for the update kernel of the previous one), under the lock so that the chain is a total order
+  // next call waits for the update kernel of the previous one). Growing the buffer, reading its address, the wait, the
+  // launches and the record all happen under ONE hold of the lock: the chain is a total order, and no other host thread
+  // can free and re-allocate the buffer (a larger generic shape) between this call's pointer read and its launches.
   std::lock_guard<std::mutex> lk(g_mutex);
+  int rc = ensure_scratch_locked(generic_scratch_bytes<R>(chunk, N, ghost));
+  if (rc) return rc;
+  R* FS = reinterpret_cast<R*>(g_state.scratch);
+  R* FL = FS + (size_t)chunk * sh.fs_stride;
   if (g_state.scratch_used) CK(cudaStreamWaitEvent(stream, g_state.scratch_free, 0));
   for (int g0 = 0; g0 < n_groups; g0 += chunk) {
     const int ng = (n_groups - g0) < chunk ? (n_groups - g0) : chunk;
@@ -368,7 +395,9 @@ int max_speed_impl(const R* U, int n_groups, int N, int ghost, double gamma, dou
   if (n_groups == 0) return 0;
   int rc = ensure_init();
   if (rc) return rc;
-  Bits* slot = reinterpret_cast<Bits*>(next_reduce_slot());
+  SlotLease lease;   // held until the value has been read back (the stream is synchronised below)
+  if (!lease.ok()) return GAMER_HYDRO_BUSY;
+  Bits* slot = reinterpret_cast<Bits*>(lease.ptr());
   CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
   const long long n_cells = (long long)n_groups * N * N * N;
   const int threads = 256;
@@ -510,7 +539,7 @@ static int step_grid_impl(const float* U, float* U_out, float* bflux, float* U_n
   if (rc) return rc;
   if (N != gh::FN || ghost != 2) return GAMER_HYDRO_UNSUPPORTED;   // the fused-halo kernel is the N = 16, ghost = 2 one
   if ((rc = ensure_init())) return rc;
-  unsigned int* slot = reinterpret_cast<unsigned int*>(max_slot ? max_slot : next_reduce_slot());
+  unsigned int* slot = reinterpret_cast<unsigned int*>(max_slot ? max_slot : sink_reduce_slot());
   CK(cudaMemsetAsync(slot, 0, sizeof(unsigned long long), stream));
   const gh::HaloGrid hg = {U_next, slot, gx, gy, gz};
   return launch_duo(U, U_out, bflux, ng, N, ghost, dt, dx, gamma, limiter, stream, &hg);
@@ -533,7 +562,9 @@ int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, in
   double vmax = 0.0;
   int rc = gamer_hydro_max_speed(U, 4, (int)ng, N, ghost, (double)gamma, &vmax, stream);   // state on entry
   if (rc) return rc;
-  unsigned long long* const slot = next_reduce_slot();   // this call's own reduction slot (calls on other streams take others)
+  SlotLease lease;   // this call's own reduction slot for all its steps (every step ends with a synchronised read)
+  if (!lease.ok()) return GAMER_HYDRO_BUSY;
+  unsigned long long* const slot = lease.ptr();
   // Default: step + ghost refill (the refill pass also accumulates the next signal-speed maximum). With the DUO path
   // selected, a fully periodic grid of 16^3 groups uses the fused-halo variant of that kernel instead: the step
   // kernel itself writes the next step's ghosted array and signal-speed maximum (ping-pong between U and a
@@ -574,11 +605,11 @@ int gamer_hydro_advance(float* U, float* U_out, float* bflux, int gx, int gy, in
         return finish(rc);
       float* tmp = cur; cur = nxt; nxt = tmp;
     } else {
-      if ((rc = gamer_hydro_step(U, U_out, bflux, (int)ng, N, ghost, dt, dx, gamma, limiter, stream))) return rc;
+      if ((rc = gamer_hydro_step(U, U_out, bflux, (int)ng, N, ghost, dt, dx, gamma, limiter, stream))) return finish(rc);
       // ghost refill fused with the signal-speed maximum of the new state (next step's dt)
       if ((rc = fill_ghosts_impl<float, unsigned int>(U_out, U, gx, gy, gz, N, ghost, bc_x, bc_y, bc_z, stream, slot,
                                                       (double)gamma)))
-        return rc;
+        return finish(rc);
     }
     unsigned int bits = 0;
     if (cudaMemcpyAsync(&bits, slot, sizeof(bits), cudaMemcpyDeviceToHost, stream) != cudaSuccess ||
@@ -813,6 +844,8 @@ const char* gamer_hydro_strerror(int code) {
     case GAMER_HYDRO_UNSUPPORTED: return "unsupported shape for the requested kernel path";
     case GAMER_HYDRO_CUDA_ERROR: return g_state.cuda_msg;
     case GAMER_HYDRO_NOT_SM100: return "device is not compute capability 10.x (sm_100a required)";
+    case GAMER_HYDRO_BUSY:
+      return "all 64 signal-speed reduction slots are leased by gamer_hydro_max_speed / gamer_hydro_advance calls in flight";
     case GAMER_HYDRO_TOO_LARGE:
       return "batch exceeds the fixed scratch array of gamer_hydro_max_speed_noalloc (65536 patch groups at most): "
              "split the batch or call gamer_hydro_max_speed";

@@ -10,7 +10,9 @@ namespace gh {
 // max over the interior cells of all groups of |vx| + |vy| + |vz| + 3 c_s (R15). U: [G][5][S][S][S] with
 // S = N + 2 ghost (ghost = 0 for U_out). The result is accumulated with an integer atomicMax on the bit pattern
 // (non-negative IEEE values order like unsigned integers; a NaN orders above them all, so a state holding NaN gives
-// a NaN maximum and the caller's dt check trips), so *out must be zeroed before the launch.
+// a NaN maximum and the caller's dt check trips), so *out must be zeroed before the launch. A cell with rho <= 0 gives
+// NaN only while its pressure expression is positive (root of a negative number); with the pressure clamped to 0 its
+// speed is <= 0 and it drops out of the maximum — the check is for NaN states, not a positivity check (R10 counts those).
 // NC, GC > 0: compile-time patch size and ghost width (the 16 / 2 of the configs: the index arithmetic becomes shifts).
 template <class R, class Bits, int NC, int GC>
 __global__ void max_speed_kernel(const R* __restrict__ U, long long n_cells, int N_rt, int ghost_rt, R gamma, Bits* out) {

@@ -55,6 +55,7 @@ def test_strerror_and_argument_validation_without_a_device():
     import paper_1007_3818_b200 as gh
     assert gh.gamer_hydro_strerror(0) == "success"
     assert "invalid" in gh.gamer_hydro_strerror(1)
+    assert "64" in gh.gamer_hydro_strerror(6) and "unknown" in gh.gamer_hydro_strerror(7)     # GAMER_HYDRO_BUSY; no code 7
     L = gh.binding.lib()
     # validation happens before any CUDA call, so these return INVALID_ARG (1) even on a box with no GPU
     assert L.gamer_hydro_step(None, None, None, -1, 16, 2, 1e-3, 1e-2, 5 / 3, 0, None) == 1

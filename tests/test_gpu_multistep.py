@@ -265,3 +265,90 @@ def test_advance_reports_a_nan_state_and_leaves_the_completed_steps_in_U():
     with pytest.raises(gh.GamerHydroError):
         gh.gamer_hydro_advance(d_U, d_out, None, _grid(w.shape), 3, 0.4, pu.f32(w.dx), limiter=w.limiter)
     assert np.isnan(gh.gamer_hydro_max_speed(d_U))
+
+
+def test_advance_keeps_its_reduction_slot_while_another_thread_reduces_hundreds_of_times():
+    """the reduction slots used to be handed out round robin modulo 64 with no owner, so 64 calls of
+    gamer_hydro_max_speed on another thread wrapped around onto the slot a running gamer_hydro_advance kept for all its
+    steps (zeroed it, or added a foreign maximum: wrong dt). Slots are now leased for the duration of the call. A
+    12-step advance on a cold field (maximum ~ 0.16) runs beside 400 max_speed calls on a hot field (maximum ~ 16) on a
+    second thread and stream: the dt sequence and the final state must be the bits of the same advance run alone."""
+    import threading
+    w = wl.config_3_cosmo(64, seed=31)
+    hot = torch.from_numpy(wl.config_2_turbulence(64, seed=4).groups()).to(DEV)
+    v_hot = gh.gamer_hydro_max_speed(hot)
+    steps = 12
+
+    def advance(out):
+        st = torch.cuda.Stream()
+        with torch.cuda.stream(st):
+            d_U = torch.from_numpy(w.groups()).to(DEV)
+            d_out = torch.empty((d_U.shape[0], 5, 16, 16, 16), dtype=torch.float32, device=DEV)
+            dts = gh.gamer_hydro_advance(d_U, d_out, None, _grid(w.shape), steps, 0.4, pu.f32(w.dx),
+                                         bc=[BC[b] for b in w.bc], limiter=w.limiter, stream=st)
+            st.synchronize()
+            out.append((dts, d_U.cpu().numpy()))
+
+    alone = []
+    advance(alone)
+    for rep in range(2):
+        both, seen, stop = [], [], threading.Event()
+
+        def hammer():
+            st = torch.cuda.Stream()
+            while not stop.is_set() or len(seen) < 400:
+                seen.append(gh.gamer_hydro_max_speed(hot, stream=st))
+
+        t1, t2 = threading.Thread(target=advance, args=(both,)), threading.Thread(target=hammer)
+        t2.start(); t1.start(); t1.join(); stop.set(); t2.join()
+        assert len(seen) >= 400 and all(v == v_hot for v in seen)             # nor did the advance disturb the hammer
+        assert both[0][0] == alone[0][0]                                      # same dt sequence, bit for bit
+        assert np.array_equal(both[0][1], alone[0][1])
+
+
+def test_generic_path_steps_of_growing_shapes_on_two_threads():
+    """launch_generic used to read the scratch address outside the lock under which another thread may
+    free and re-allocate it for a larger shape. Two host threads step generic shapes (N = 8 / ghost 2 and N = 12 /
+    ghost 3: the second needs the larger scratch, and both start before it exists) on their own streams; every result
+    must be the bits of the same call made alone."""
+    import threading
+    shapes = [(8, 2, 40), (12, 3, 24)]
+    rng = np.random.default_rng(77)
+    data = []
+    for N, ghost, n in shapes:
+        S = N + 2 * ghost
+        U = np.empty((n, 5, S, S, S), dtype=np.float32)
+        U[:, 0] = rng.uniform(0.5, 2.0, (n, S, S, S))
+        U[:, 1:4] = rng.uniform(-0.3, 0.3, (n, 3, S, S, S)) * U[:, :1]
+        U[:, 4] = rng.uniform(1.0, 2.0, (n, S, S, S)) / (G - 1.0) + 0.5 * (U[:, 1:4] ** 2).sum(axis=1) / U[:, 0]
+        data.append(torch.from_numpy(U).to(DEV))
+    dt, dx = pu.f32(2e-3), pu.f32(1.0 / 32)
+
+    def step(k, st, out):
+        N, ghost, n = shapes[k]
+        with torch.cuda.stream(st):
+            o = torch.full((n, 5, N, N, N), float("nan"), dtype=torch.float32, device=DEV)
+            bf = torch.full((n, 6, 5, N, N), float("nan"), dtype=torch.float32, device=DEV)
+            gh.gamer_hydro_step(data[k], o, bf, n, N, ghost, dt, dx, G, gh.MINMOD, stream=st)
+            st.synchronize()
+            out.append((o.cpu().numpy(), bf.cpu().numpy()))
+
+    gh.gamer_hydro_free()                                       # start without any scratch: the first calls grow it
+    conc = [[], []]
+
+    def loop(k):
+        st = torch.cuda.Stream()
+        for _ in range(20):
+            step(k, st, conc[k])
+
+    th = [threading.Thread(target=loop, args=(k,)) for k in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    for k in range(2):
+        ref = []
+        step(k, torch.cuda.Stream(), ref)
+        assert np.isfinite(ref[0][0]).all() and np.isfinite(ref[0][1]).all()
+        for o, bf in conc[k]:
+            assert np.array_equal(o, ref[0][0]) and np.array_equal(bf, ref[0][1])
