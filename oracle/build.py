@@ -29,7 +29,7 @@ def build(force: bool = False) -> str:
     return LIB
 
 
-RTVD_SOURCES = ["rtvd_oracle_capi.cpp", "rtvd_oracle.hpp"]
+RTVD_SOURCES = ["rtvd_oracle_capi.cpp", "rtvd_oracle.hpp", "counting_real.hpp"]
 RTVD_LIB = os.path.join(HERE, "librtvd_oracle.so")
 
 

@@ -32,8 +32,24 @@ def lib():
         L.rtvd_oracle_vanleer.argtypes = [C.c_double, C.c_double]
         L.rtvd_oracle_flux_and_speed.restype = None
         L.rtvd_oracle_flux_and_speed.argtypes = [_dp, C.c_int, C.c_double, _dp, _dp]
+        L.rtvd_oracle_count_flops.restype = None
+        L.rtvd_oracle_count_flops.argtypes = [_dp, C.c_int, C.c_double, C.c_double, C.c_double, C.c_int,
+                                              C.POINTER(C.c_ulonglong)]
         _lib = L
     return _lib
+
+
+def count_flops(U_in, N, dt, dx, gamma, sweep):
+    """Algorithmic FLOPs of one step on ONE group U_in [5][N+6][N+6][N+6]: the oracle text run with a counting scalar
+    (oracle/counting_real.hpp). Returns dict(add, mul, div, sqrt, minmax, total, per_cell); per_cell = total / N^3."""
+    U = np.ascontiguousarray(U_in, dtype=np.float64)
+    assert U.shape == (5, N + 6, N + 6, N + 6), U.shape
+    c = (C.c_ulonglong * 5)()
+    lib().rtvd_oracle_count_flops(_ptr(U), N, float(dt), float(dx), float(gamma), int(sweep), c)
+    d = dict(zip(("add", "mul", "div", "sqrt", "minmax"), (int(v) for v in c)))
+    d["total"] = sum(d.values())
+    d["per_cell"] = d["total"] / float(N ** 3)
+    return d
 
 
 def step_groups(U_in, N, dt, dx, gamma, sweep, n_threads=0):

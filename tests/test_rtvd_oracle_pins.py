@@ -173,3 +173,28 @@ def test_one_dimensional_data_stay_one_dimensional_in_3d():
         ref = R.sweep_line(np.concatenate([line[-3:], line, line[:3]]), 0, dt, dx, G)[3:-3]
         assert np.array_equal(out[2], np.zeros_like(out[2])) and np.array_equal(out[3], np.zeros_like(out[3]))
         assert np.array_equal(out[:, 2, 5, :], ref.T) and np.array_equal(out[:, 7, 0, :], ref.T)
+
+
+def test_flop_tally_matches_a_hand_count_of_the_oracle_text():
+    """The roofline numerator of bench.py's relaxing-TVD leg (RTVD_FLOPS_PER_CELL) is the oracle text run with a counting
+    scalar. Pin: the count typed out here by hand from the text of sweep_line, per line of L cells, convention of
+    oracle/counting_real.hpp (add = sub = mul = div = sqrt = 1; abs, negate, compare, select = 0):
+      flux_and_speed 21 per cell (v 1; ke 7; P 3; F 6; c 4) + the split fluxes 2 x 3 x 5 = 30   -> 51 per cell
+      half step: 51 L + 5 (L-1) first-order face fluxes + 20 (L-2) for the half-step state
+      full step: 51 (L-2) + 95 (L-5) limited face fluxes (19 per variable) + 15 (L-6) update; 1 for lambda = dt/dx
+    over the 22^2 + 22*16 + 16^2 = 1092 lines a 16^3 group's three sweeps touch (RT5: the range shrinks after a sweep).
+    Opposite-sign differences skip the 4 operations of the van Leer quotient, so the tally may sit slightly below."""
+    import bench
+    L, N = 22, 16
+    per_line = 51 * L + 5 * (L - 1) + 20 * (L - 2) + 51 * (L - 2) + 95 * (L - 5) + 15 * (L - 6) + 1
+    lines = L * L + L * N + N * N
+    hand = per_line * lines / float(N ** 3)
+    assert per_line == 4503 and lines == 1092 and abs(hand - 1200.5) < 0.05
+    z, y, x = np.meshgrid(*(np.arange(L, dtype=np.float64),) * 3, indexing="ij")
+    ramp = 1.0 + 0.01 * (x + 2 * y + 3 * z)          # monotone along every axis: (almost) every limiter active
+    U = wl.prim_box_to_cons(ramp, 0.1 * ramp, -0.2 * ramp, 0.3 * ramp, 2.0 * ramp)
+    for sweep in (0, 1):
+        c = R.count_flops(U, N, 1e-3, 1 / 16, G, sweep)
+        assert c["sqrt"] == lines * (2 * L - 2) and c["minmax"] == 0
+        assert 0.999 * hand <= c["per_cell"] <= hand, (c, hand)
+        assert abs(bench.RTVD_FLOPS_PER_CELL - c["per_cell"]) <= 1.0, (bench.RTVD_FLOPS_PER_CELL, c["per_cell"])
