@@ -568,3 +568,24 @@ def test_flop_tally_band():
     assert 0.85 * 925 <= c0["per_cell"] <= 1.15 * 925, c0
     assert c1["per_cell"] > c0["per_cell"]
     assert c0["sqrt"] == 3 * 13056 and c0["minmax"] == 15 * 5632
+
+
+def test_sedov_golden_constants_are_rederived_by_the_committed_calculator():
+    """tests/golden/sedov_xi0.txt (used by P15 and the cfg 4 tests for the shock radius) against tests/sedov_taylor.py:
+    the self-similar ODEs integrated inward from the strong-shock conditions and normalised by the energy integral
+    (SURVEY.md Appendix A). gamma = 1.4 gives the textbook 1.033; a closed form exists for no gamma, but the integrated
+    profile must show the flat central pressure of Taylor's solution, P(0) / P(1) = 0.366 for gamma = 1.4."""
+    import sedov_taylor as st
+    golden = {}
+    with open(os.path.join(os.path.dirname(__file__), "golden", "sedov_xi0.txt")) as f:
+        for line in f:
+            if line.strip() and not line.startswith("#"):
+                k, v = line.split()
+                golden[k] = float(v)
+    assert abs(st.xi0(5.0 / 3.0) - golden["gamma_5_3"]) <= 1e-5
+    assert abs(st.xi0(1.4) - golden["gamma_1_4"]) <= 1e-5
+    assert abs(st.xi0(1.4) - 1.033) <= 5e-4                              # the value every textbook prints
+    assert abs(st.xi0(1.4, lam_min=1e-2) - st.xi0(1.4, lam_min=1e-4)) <= 1e-9   # the inner cut-off does not matter
+    sol = st.profiles(1.4)
+    assert abs(np.exp(sol.y[2, -1] - sol.y[2, 0]) - 0.366) <= 2e-3       # central over post-shock pressure
+    assert sol.y[1, -1] < np.log(1e-6)                                   # the centre is evacuated
