@@ -466,8 +466,25 @@ def main():
         torch.cuda.synchronize()
         ms3 = e0.elapsed_time(e1) / 10
         c3 = n3 * N ** 3
+        # parity spot-check on the input just timed (as the headline has): 64 groups spread over the batch, one step in
+        # either sweep order against the fp64 oracle (all 4096 groups: tests/test_gpu_rtvd.py)
+        rtvd_parity = None
+        if not args.no_cpu_baseline:
+            from oracle import rtvd_oracle as RO
+            from harness import metrics as hm
+            pick = np.arange(0, n3, max(1, n3 // 64))[:64]
+            sub = g3[torch.from_numpy(pick).to(dev)].contiguous()
+            rtvd_parity = 0.0
+            for sw in (0, 1):
+                o_s = torch.empty((len(pick), 5, N, N, N), dtype=torch.float32, device=dev)
+                gh.gamer_rtvd_step(sub, o_s, len(pick), N, 3, dt3, dx3, w2.gamma, sw, stream=stream)
+                torch.cuda.synchronize()
+                ref_s, _ = RO.step_groups(sub.cpu().numpy(), N, dt3, dx3, w2.gamma, sw)
+                rtvd_parity = max(rtvd_parity, float(hm.max_rel_err(o_s.cpu().numpy(), ref_s, w2.gamma)))
         rtvd = {"value": c3 / (ms3 * 1e-3), "unit": UNIT, "ms_per_step": ms3, "groups": n3, "ghost": 3,
                 "api": "gamer_rtvd_step (x,y,z / z,y,x sweeps alternating)", "kernel": "gh::rtvd_kernel",
+                "parity_max_rel_err_on_sample": rtvd_parity, "parity_tolerance": 1e-4,
+                "parity_sample": "64 of the timed groups, both sweep orders, vs oracle/rtvd_oracle.hpp",
                 "roofline": {"bound": "alu", "flops_per_cell_update": RTVD_FLOPS_PER_CELL,
                              "achieved": RTVD_FLOPS_PER_CELL * c3 / (ms3 * 1e-3) / 1e12, "peak": ALU_PEAK_TFLOPS,
                              "unit": "TFLOP/s", "frac": RTVD_FLOPS_PER_CELL * c3 / (ms3 * 1e-3) / 1e12 / ALU_PEAK_TFLOPS,

@@ -96,3 +96,45 @@ def test_argument_errors():
         gh.gamer_rtvd_step(torch.ones((1, 5, 24, 24, 24), device=DEV), out, 1, 16, 4, 1e-3, 1e-2, G, 0)
     gh.gamer_rtvd_step(torch.zeros((0, 5, 22, 22, 22), device=DEV), torch.zeros((0, 5, 16, 16, 16), device=DEV), 0, 16, 3,
                        1e-3, 1e-2, G, 0)           # empty batch is a no-op
+
+
+def _nonpositive(U):
+    """Cells with rho <= 0 or P <= 0 in a [..., 5, z, y, x]-like array (fp64 arithmetic)."""
+    U = np.asarray(U, dtype=np.float64)
+    rho, mx, my, mz, E = (np.take(U, q, axis=-4) for q in range(5))
+    P = (G - 1.0) * (E - 0.5 * (mx * mx + my * my + mz * mz) / rho)
+    return int(((rho <= 0) | (P <= 0)).sum())
+
+
+def test_the_field_the_bench_times_all_4096_groups_both_sweep_orders_and_ten_steps():
+    """bench.py's relaxing-TVD leg runs on the Mach-30 field of configs[3] at 256^3 cut
+    with three ghost cells (4096 groups, 28 per persistent CTA) — this is that input (same recipe, seed, dt and dx as
+    bench.py), ALL 4096 groups element by element against the fp64 oracle: one step in either sweep order within 1e-4,
+    then ten steps with alternating order within 1e-3. fp32 pressure from E - ke at Mach 30 with the max(P, 0) clamp of
+    RT6 is where a relaxing-TVD kernel could drift from its oracle. Output finite; non-positive cells are counted on
+    both sides and must agree (RT6: no floors anywhere, so the count is part of the result)."""
+    w = wl.config_3_cosmo(256, seed=3)
+    dx = pu.f32(w.dx)
+    grp = wl.cut_groups(w.U, w.bc, ghost=3)
+    assert grp.shape == (4096, 5, 22, 22, 22)
+    dt = pu.f32(w.dt())
+    for sweep in (0, 1):
+        out = run_gpu(grp, dt, dx, sweep)
+        ref, _ = R.step_groups(grp, 16, dt, dx, G, sweep)
+        assert np.isfinite(out).all()
+        err = metrics.max_rel_err(out, ref, G)
+        bad_gpu, bad_ref = _nonpositive(out), _nonpositive(ref)
+        print("rtvd cfg3 256^3 sweep %d: max rel err %.3e, non-positive cells gpu %d / oracle %d" % (sweep, err, bad_gpu, bad_ref))
+        assert err <= TOL1, (sweep, err)
+        assert bad_gpu == bad_ref
+    Ug, Uo = w.U.copy(), w.U.astype(np.float64)
+    for s in range(10):
+        dt = wl.cfl_dt(Ug, w.dx, 0.5)
+        Ug = wl.assemble_box(run_gpu(wl.cut_groups(Ug, w.bc, ghost=3), dt, dx, s % 2), w.shape)
+        o, _ = R.step_groups(wl.cut_groups(Uo, w.bc, ghost=3), 16, dt, dx, G, s % 2)
+        Uo = wl.assemble_box(o, w.shape)
+        assert np.isfinite(Ug).all(), s
+    err10 = metrics.max_rel_err(Ug[None], Uo[None], G)
+    print("rtvd cfg3 256^3 ten alternating steps: max rel err %.3e, non-positive cells gpu %d / oracle %d"
+          % (err10, _nonpositive(Ug), _nonpositive(Uo)))
+    assert err10 <= TOL10, err10

@@ -100,3 +100,54 @@ def test_step_ex_with_everything_off_is_the_plain_step_bit_for_bit():
         run_ex(g, dt, dx, 1, 4, False)                                   # unknown flag bit
     with pytest.raises(gh.GamerHydroError):
         pu.run_gpu(g, dt, dx, G, 3)                                      # unknown limiter
+
+
+# ---- every limiter / variant instantiation streamed through its persistent ring: the tests
+# above use 3-4 groups, one per CTA, so zpair_kernel<2>, duo_kernel<2> and the fused_kernel<..., VAR = true>
+# instantiations never recycled a ring slot in any test. 2 * 148 + 37 groups = three groups on most CTAs, ragged tail.
+N_RING = 2 * 148 + 37
+SAMPLE = np.r_[0:3, 147:150, 295:298, N_RING - 3:N_RING]
+
+
+@pytest.mark.parametrize("path", [gh.PATH_FUSED, gh.PATH_FUSED_DUO, gh.PATH_FUSED_SCALAR])
+def test_mc_limiter_streams_many_groups_through_every_fused_ring(path):
+    g = wl.random_groups(N_RING, seed=305)
+    dt, dx = pu.f32(2e-3), pu.f32(1 / 16)
+    out, bf, _ = pu.run_gpu(g, dt, dx, G, gh.MC, path=path)
+    r, _ = O.step_groups_ex(g[SAMPLE], 16, 2, dt, dx, G, gh.MC)
+    assert metrics.max_rel_err(out[SAMPLE], r.U_out, G) <= 1e-4
+    assert float(metrics.bflux_errors(bf[SAMPLE], r.bflux, r.U_out, G).max()) <= 1e-3
+    one, bf1, _ = pu.run_gpu(g[150:151], dt, dx, G, gh.MC, path=path)
+    assert np.array_equal(one[0], out[150]) and np.array_equal(bf1[0], bf[150])      # independent of the batch
+    for _ in range(10):                                                              # and of the launch
+        o2, b2, _ = pu.run_gpu(g, dt, dx, G, gh.MC, path=path)
+        assert np.array_equal(o2, out) and np.array_equal(b2, bf)
+
+
+@pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-4), (np.float64, 1e-11)])
+@pytest.mark.parametrize("flags", [1, 2, 3])
+def test_variant_kernels_stream_many_groups_through_their_ring(flags, dtype, tol):
+    """The scalar fused kernel with VAR = true (entropy fix, HLLE fallback, mid-plane fluxes), fp32 and fp64, on the
+    supersonic random states of the test above. Element-by-element parity on the sampled groups in fp64 for every flag
+    and in fp32 for the entropy fix (a continuous change of the flux); the fp32 HLLE switch is a discontinuous decision
+    whose marginal faces may flip (the 4-group test above accounts for them), so for flags 2 and 3 in fp32 this test
+    checks what does not depend on them: bits independent of the batch and of the launch, finite output."""
+    g = wl.random_groups(N_RING, seed=306, mach=2.0, contrast=0.8, dtype=dtype)
+    dt, dx = (pu.f32(5e-4), pu.f32(1 / 16)) if dtype == np.float32 else (5e-4, 1 / 16)
+    out, bf, mf = run_ex(g, dt, dx, 1, flags, True)
+    assert np.isfinite(out).all() and np.isfinite(bf).all() and np.isfinite(mf).all()
+    if dtype == np.float64 or flags == 1:
+        r, mfo = O.step_groups_ex(g[SAMPLE], 16, 2, dt, dx, G, 1, flags, want_midflux=True)
+        assert metrics.max_rel_err(out[SAMPLE], r.U_out, G) <= tol
+        assert float(metrics.bflux_errors(bf[SAMPLE], r.bflux, r.U_out, G).max()) <= 10 * tol
+        rho, E, a = metrics._scales(r.U_out, G)                      # mid-plane flux scale, as in test_midplane_fluxes
+        for ax, sl in enumerate([np.s_[:, :, :, 8], np.s_[:, :, 8, :], np.s_[:, 8, :, :]]):
+            base = rho[sl] * a[sl]
+            sc = [base, base * a[sl], base * a[sl], base * a[sl], base * a[sl] * a[sl]]
+            for q in range(5):
+                assert (np.abs(mf[SAMPLE][:, ax, q] - mfo[:, ax, q]) / sc[q]).max() <= 10 * tol
+    o1, b1, m1 = run_ex(g[150:151], dt, dx, 1, flags, True)
+    assert np.array_equal(o1[0], out[150]) and np.array_equal(b1[0], bf[150]) and np.array_equal(m1[0], mf[150])
+    for _ in range(10):
+        o2, b2, m2 = run_ex(g, dt, dx, 1, flags, True)
+        assert np.array_equal(o2, out) and np.array_equal(b2, bf) and np.array_equal(m2, mf)
