@@ -360,11 +360,11 @@ def main():
     hbm_gbs = BYTES_PER_CELL * cells / (ms_launch * 1e-3) / 1e9
     traffic, traffic_src = None, None
     try:
-        with open(os.path.join(ROOT, "profiles", "r2b_traffic_bytes_per_launch.txt")) as f:
+        with open(os.path.join(ROOT, "profiles", "r3_traffic_bytes_per_launch.txt")) as f:
             tj = json.load(f)
             if tj.get("n_groups") == G and args.path in ("auto", "fused"):
                 traffic = tj["dram_bytes_read_plus_write"]
-                traffic_src = "ncu --set full capture, profiles/r2b_traffic_bytes_per_launch.txt (commit %s)" % tj.get("commit")
+                traffic_src = "ncu --set full capture, profiles/r3_traffic_bytes_per_launch.txt (commit %s)" % tj.get("commit")
     except Exception:
         pass
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
@@ -389,11 +389,14 @@ def main():
         # run against the issue cost of the kernel's executed instruction mix (profiles/r2b_README.md: packed f32x2 = 2
         # clocks, 3 with three distinct source pairs; measured by harness/issue_microbench.py)
         sched_clocks = ms_launch * 1e-3 * SM_MAX_GHZ * 1e9 * SM_COUNT * 4 * 32 / cells
-        roofline["issue"] = {"scheduler_clocks_per_cell_update": sched_clocks,
-                             "issue_cost_of_instruction_mix": ISSUE_COST_PER_CELL,
-                             "frac_of_issue_bound": ISSUE_COST_PER_CELL / sched_clocks,
-                             "clocks_at_target_frac": FLOPS_PER_CELL[0] / (2 * 0.60),
-                             "source": "profiles/r2b_README.md, harness/issue_microbench.py"}
+        roofline["issue_model"] = {"kind": "MODEL, not a counter: executed instruction mix (profiles/r3_zpair_opcode_mix.csv) "
+                                           "x per-opcode issue cost (harness/issue_microbench.py); ncu's own counter is "
+                                           "smsp__issue_active in profiles/r3_zpair_kernel_ncu_full.csv",
+                                   "scheduler_clocks_per_cell_update": sched_clocks,
+                                   "modelled_issue_cost_of_instruction_mix": ISSUE_COST_PER_CELL,
+                                   "modelled_frac_of_issue_bound": ISSUE_COST_PER_CELL / sched_clocks,
+                                   "clocks_at_target_frac": FLOPS_PER_CELL[0] / (2 * 0.60),
+                                   "source": "profiles/r2b_README.md, harness/issue_microbench.py"}
 
     # ---- cpu_baseline: the oracle on a bounded sample of the same workload (+ parity spot-check)
     cpu = None
