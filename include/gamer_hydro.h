@@ -228,6 +228,15 @@ int gamer_hydro_status(unsigned long long* guard_cells, unsigned long long* nonp
  * in chunks (every chunk would mark the map from g = 0 again). */
 int gamer_hydro_set_guard_map(unsigned char* device_map);
 
+/* The same aid for the HLLE fallback of gamer_hydro_step_ex (GAMER_HYDRO_FLAG_HLLE_FALLBACK is a discontinuous switch:
+ * a face whose intermediate state is marginal can take the other branch in fp32 than in the fp64 oracle). With
+ * device_map != NULL every later step_ex call marks the faces that took the HLLE branch:
+ * device_map[g][axis][k][j][i] = 1, unsigned char [n_groups][3][N+1][N+1][N+1] in DEVICE memory, owned and zeroed by the
+ * caller; the face is the one on the lower side of cell (i, j, k) along the axis (index N = the upper outer face).
+ * NULL (the default) switches it off. Process-global, synchronises the device; same caveat about
+ * gamer_hydro_step_host as the guard map. */
+int gamer_hydro_set_hlle_map(unsigned char* device_map);
+
 /* Forces a kernel path (tests, benchmarking); GAMER_HYDRO_PATH_AUTO restores the default. */
 int gamer_hydro_set_path(int path);
 

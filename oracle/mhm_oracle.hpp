@@ -265,12 +265,17 @@ inline void roe_flux(const T UL[5], const T UR[5], T gamma, int d, T F[5], int f
 //   midflux (nullable): the fluxes on the three MID-planes of the box (the faces at index n/2 - 1/2 along each axis,
 //          between the two halves a group of 2 x 2 x 2 patches consists of; reading R12b): [3][5][.][.] in the
 //          in-face layout of the outer faces of the same axis, x mid-plane first. Needs even nx, ny, nz.
+//   hlle_faces (nullable): [3][nz+1][ny+1][nx+1] bytes, 1 where the face on the LOWER side of cell (i,j,k) along axis d
+//          took the HLLE branch (flags & HLLE_FALLBACK): like `guard`, a diagnostic for the parity harness (a face whose
+//          intermediate state is marginal can take the other branch in fp32), not used here. Entries of faces that do
+//          not exist (index nx along y or z, ...) are left untouched.
 // A patch group is the special case nx = ny = nz = N (O8: the per-group and global forms are the same text).
 struct StepStats { unsigned long long guard_cells = 0, nonpositive_out = 0; };
 
 template <class T>
 StepStats step_box(const T* U_in, int nx, int ny, int nz, int g, T dt, T dx, T gamma, int limiter,
-                   T* U_out, T* bflux, unsigned char* guard, double* margin, int flags = 0, T* midflux = nullptr) {
+                   T* U_out, T* bflux, unsigned char* guard, double* margin, int flags = 0, T* midflux = nullptr,
+                   unsigned char* hlle_faces = nullptr) {
   StepStats stats;
   const int sx = nx + 2 * g, sy = ny + 2 * g, sz = nz + 2 * g;
   const size_t plane = (size_t)sx * sy, vol = plane * sz;
@@ -393,7 +398,10 @@ StepStats step_box(const T* U_in, int nx, int ny, int nz, int g, T dt, T dx, T g
             UL[q] = ub(i - e[d][0], j - e[d][1], k - e[d][2], d, 1, q);  // left cell's '+' state
             UR[q] = ub(i, j, k, d, 0, q);                                // right cell's '-' state
           }
-          roe_flux(UL, UR, gamma, d, Ff, flags);
+          bool took_hlle = false;
+          roe_flux(UL, UR, gamma, d, Ff, flags, &took_hlle);
+          if (hlle_faces)   // diagnostic for the parity harness: which faces took the HLLE branch (R8c)
+            hlle_faces[(((size_t)d * (nz + 1) + k) * (ny + 1) + j) * (nx + 1) + i] = took_hlle ? 1 : 0;
           for (int q = 0; q < 5; ++q) fl(d, q, i, j, k) = Ff[q];
         }
 

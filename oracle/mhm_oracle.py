@@ -49,7 +49,7 @@ def lib():
                                              _u64p]
         L.mhm_oracle_step_groups_ex.restype = C.c_int
         L.mhm_oracle_step_groups_ex.argtypes = [_dp, C.c_int, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double,
-                                                C.c_int, C.c_int, _dp, _dp, _dp, _u8p, _u64p, C.c_int]
+                                                C.c_int, C.c_int, _dp, _dp, _dp, _u8p, _u64p, C.c_int, _u8p]
         L.mhm_oracle_roe_flux_ex.restype = C.c_int
         L.mhm_oracle_roe_flux_ex.argtypes = [_dp, _dp, C.c_double, C.c_int, C.c_int, _dp]
         _lib = L
@@ -88,9 +88,11 @@ def step_groups(U_in, N, ghost, dt, dx, gamma, limiter, want_bflux=True, want_gu
 ENTROPY_FIX, HLLE_FALLBACK = 1, 2
 
 
-def step_groups_ex(U_in, N, ghost, dt, dx, gamma, limiter, flags=0, want_midflux=False, n_threads=0):
+def step_groups_ex(U_in, N, ghost, dt, dx, gamma, limiter, flags=0, want_midflux=False, n_threads=0, want_hlle=False):
     """step_groups with the robustness variants: limiter 2 = MC, flags = ENTROPY_FIX |
-    HLLE_FALLBACK, optional mid-plane fluxes [G][3][5][N][N]. Returns (StepResult, midflux or None)."""
+    HLLE_FALLBACK, optional mid-plane fluxes [G][3][5][N][N]. Returns (StepResult, midflux or None). With want_hlle the
+    result carries .hlle, uint8 [G][3][N+1][N+1][N+1]: 1 where the face on the lower side of cell (i,j,k) along axis d
+    took the HLLE branch (index [g][d][k][j][i])."""
     U = np.ascontiguousarray(U_in, dtype=np.float64)
     S = N + 2 * ghost
     assert U.ndim == 5 and U.shape[1:] == (5, S, S, S), U.shape
@@ -100,10 +102,13 @@ def step_groups_ex(U_in, N, ghost, dt, dx, gamma, limiter, flags=0, want_midflux
     mf = np.empty((G, 3, 5, N, N), dtype=np.float64) if want_midflux else None
     gd = np.zeros((G, N + 2, N + 2, N + 2), dtype=np.uint8)
     stats = np.zeros(2, dtype=np.uint64)
+    hl = np.zeros((G, 3, N + 1, N + 1, N + 1), dtype=np.uint8) if want_hlle else None
     used = lib().mhm_oracle_step_groups_ex(_ptr(U, _dp), G, N, ghost, float(dt), float(dx), float(gamma), int(limiter),
                                            int(flags), _ptr(out, _dp), _ptr(bf, _dp), _ptr(mf, _dp), _ptr(gd, _u8p),
-                                           _ptr(stats, _u64p), int(n_threads))
-    return StepResult(out, bf, gd, None, int(stats[0]), int(stats[1]), int(used)), mf
+                                           _ptr(stats, _u64p), int(n_threads), _ptr(hl, _u8p))
+    r = StepResult(out, bf, gd, None, int(stats[0]), int(stats[1]), int(used))
+    r.hlle = hl
+    return r, mf
 
 
 def roe_flux_ex(UL, UR, gamma, d, flags):

@@ -52,9 +52,11 @@ int mhm_oracle_step_groups(const double* U_in, int n_groups, int N, int ghost, d
 // The same with the robustness variants: flags = RiemannFlags, midflux [n_groups][3][5][N][N] or NULL.
 int mhm_oracle_step_groups_ex(const double* U_in, int n_groups, int N, int ghost, double dt, double dx, double gamma,
                               int limiter, int flags, double* U_out, double* bflux, double* midflux,
-                              unsigned char* guard, unsigned long long* stats_out, int n_threads) {
+                              unsigned char* guard, unsigned long long* stats_out, int n_threads,
+                              unsigned char* hlle_faces) {   // hlle_faces: [n_groups][3][N+1][N+1][N+1] or NULL
   const size_t S = (size_t)N + 2 * ghost;
   const size_t in_sz = 5 * S * S * S, out_sz = (size_t)5 * N * N * N, bf_sz = (size_t)30 * N * N, mf_sz = (size_t)15 * N * N;
+  const size_t h_sz = (size_t)3 * (N + 1) * (N + 1) * (N + 1);
   const size_t g_sz = (size_t)(N + 2) * (N + 2) * (N + 2);
   unsigned long long gc = 0, npo = 0;
   int used = 1;
@@ -66,7 +68,8 @@ int mhm_oracle_step_groups_ex(const double* U_in, int n_groups, int N, int ghost
   for (int g = 0; g < n_groups; ++g) {
     StepStats st = step_box<double>(U_in + g * in_sz, N, N, N, ghost, dt, dx, gamma, limiter, U_out + g * out_sz,
                                     bflux ? bflux + g * bf_sz : nullptr, guard ? guard + g * g_sz : nullptr, nullptr,
-                                    flags, midflux ? midflux + g * mf_sz : nullptr);
+                                    flags, midflux ? midflux + g * mf_sz : nullptr,
+                                    hlle_faces ? hlle_faces + g * h_sz : nullptr);
     gc += st.guard_cells;
     npo += st.nonpositive_out;
   }

@@ -22,7 +22,7 @@ EXPORTS = ["gamer_hydro_alloc", "gamer_hydro_free", "gamer_hydro_step", "gamer_h
            "gamer_hydro_step_host", "gamer_hydro_status", "gamer_hydro_set_path", "gamer_hydro_launch_count",
            "gamer_hydro_strerror", "gamer_hydro_max_speed", "gamer_hydro_fill_ghosts", "gamer_hydro_advance",
            "gamer_hydro_step_grid", "gamer_hydro_set_guard_map", "gamer_rtvd_step", "gamer_hydro_step_ex", "gamer_hydro_step_ex_f64",
-           "gamer_hydro_max_speed_noalloc", "gamer_hydro_max_speed_noalloc_limit"]
+           "gamer_hydro_max_speed_noalloc", "gamer_hydro_max_speed_noalloc_limit", "gamer_hydro_set_hlle_map"]
 BC_PERIODIC, BC_OUTFLOW = 0, 1
 
 
@@ -53,6 +53,7 @@ def lib():
         L.gamer_hydro_step_grid.argtypes = [vp, vp, vp, vp, i, i, i, i, i, f, f, f, i, vp]
         L.gamer_hydro_advance.argtypes = [vp, vp, vp, i, i, i, i, i, i, i, i, i, f, f, f, i, vp, vp]
         L.gamer_hydro_set_guard_map.argtypes = [vp]
+        L.gamer_hydro_set_hlle_map.argtypes = [vp]
         L.gamer_rtvd_step.argtypes = [vp, vp, i, i, i, f, f, f, i, vp]
         L.gamer_hydro_step_ex.argtypes = [vp, vp, vp, vp, i, i, i, f, f, f, i, i, vp]
         L.gamer_hydro_step_ex_f64.argtypes = [vp, vp, vp, vp, i, i, i, d, d, d, i, i, vp]
@@ -298,6 +299,15 @@ def gamer_hydro_set_guard_map(device_map):
                                        device_map.is_contiguous()):
         raise GamerHydroError("guard map must be a contiguous CUDA uint8 tensor")
     _check(lib().gamer_hydro_set_guard_map(device_map.data_ptr() if device_map is not None else None))
+
+
+def gamer_hydro_set_hlle_map(device_map):
+    """device_map: zeroed uint8 CUDA tensor [n_groups][3][N+1][N+1][N+1] that later gamer_hydro_step_ex calls mark with
+    the faces that took the HLLE branch, or None to switch the export off."""
+    if device_map is not None and not (device_map.is_cuda and device_map.dtype == torch.uint8 and
+                                       device_map.is_contiguous()):
+        raise GamerHydroError("HLLE map must be a contiguous CUDA uint8 tensor")
+    _check(lib().gamer_hydro_set_hlle_map(device_map.data_ptr() if device_map is not None else None))
 
 
 def gamer_hydro_launch_count():

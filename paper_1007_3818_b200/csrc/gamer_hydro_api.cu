@@ -334,7 +334,7 @@ int launch_generic(const R* U_in, R* U_out, R* bflux, int n_groups, int N, int g
     if (limiter == 0) gh::predict_kernel<R, 0><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
     else if (limiter == 1) gh::predict_kernel<R, 1><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
     else gh::predict_kernel<R, 2><<<gp, 128, 0, stream>>>(in, FS, sh, c, g_state.status, (long long)g0);
-    gh::flux_kernel<R><<<gf, 128, 0, stream>>>(FS, FL, bf, sh, c, flags, mf);
+    gh::flux_kernel<R><<<gf, 128, 0, stream>>>(FS, FL, bf, sh, c, flags, mf, (long long)g0);
     gh::update_kernel<R><<<gu, 128, 0, stream>>>(in, FL, out, sh, c, g_state.status);
     g_launches.fetch_add(3);
   }
@@ -710,6 +710,14 @@ int gamer_hydro_set_guard_map(unsigned char* device_map) {
   if (rc) return rc;
   CK(cudaDeviceSynchronize());
   CK(cudaMemcpyToSymbol(gh::gh_guard_map, &device_map, sizeof(device_map)));
+  return 0;
+}
+
+int gamer_hydro_set_hlle_map(unsigned char* device_map) {
+  int rc = ensure_init();
+  if (rc) return rc;
+  CK(cudaDeviceSynchronize());
+  CK(cudaMemcpyToSymbol(gh::gh_hlle_map, &device_map, sizeof(device_map)));
   return 0;
 }
 

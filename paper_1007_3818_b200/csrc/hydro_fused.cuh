@@ -263,7 +263,9 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         R L[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) L[q] = xs[q * FNT + t_xl];
-        roe_flux<R, 0, Fast>(L, Wf[0][0], c, Fx, flags);
+        bool hl0 = false;
+        roe_flux<R, 0, Fast>(L, Wf[0][0], c, Fx, flags, VAR ? &hl0 : nullptr);
+        if (VAR && hl0) mark_hlle(g, FN, 0, i, j, k);
         if (VAR && mfg && i == FN / 2) {
 #pragma unroll
           for (int q = 0; q < 5; ++q) mfg[(q * FN + k) * FN + j] = Fx[q];
@@ -280,7 +282,9 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         R L[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) L[q] = ys[q * FNT + t_yl];
-        roe_flux<R, 1, Fast>(L, Wf[1][0], c, Fy, flags);
+        bool hl1 = false;
+        roe_flux<R, 1, Fast>(L, Wf[1][0], c, Fy, flags, VAR ? &hl1 : nullptr);
+        if (VAR && hl1) mark_hlle(g, FN, 1, i, j, k);
         if (VAR && mfg && j == FN / 2) {
 #pragma unroll
           for (int q = 0; q < 5; ++q) mfg[((5 + q) * FN + k) * FN + i] = Fy[q];
@@ -297,7 +301,9 @@ __global__ void __launch_bounds__(FNT, sizeof(R) == 4 ? FMINB : 1)
         R zplus[5];
 #pragma unroll
         for (int q = 0; q < 5; ++q) zplus[q] = zs[q * FNT + t];
-        roe_flux<R, 2, Fast>(zplus, Wf[2][0], c, Fz, flags);
+        bool hl2 = false;
+        roe_flux<R, 2, Fast>(zplus, Wf[2][0], c, Fz, flags, VAR ? &hl2 : nullptr);
+        if (VAR && hl2) mark_hlle(g, FN, 2, i, j, k);
         if (VAR && mfg && k == FN / 2) {
 #pragma unroll
           for (int q = 0; q < 5; ++q) mfg[((10 + q) * FN + j) * FN + i] = Fz[q];

@@ -74,7 +74,7 @@ __global__ void __launch_bounds__(128) predict_kernel(const R* __restrict__ U_in
 template <class R, int n>
 __device__ __forceinline__ void flux_face(const R* __restrict__ FSg, R* __restrict__ FLg, R* __restrict__ bf,
                                           const GenericShape& sh, const GasConst<R>& c, int i, int j, int k, int flags,
-                                          R* __restrict__ mf) {
+                                          R* __restrict__ mf, long long g) {
   // face on the lower side of cell (i,j,k) along axis n; i in [0, N] along n
   const int E = sh.E, N = sh.N;
   const long long ev = (long long)E * E * E;
@@ -87,7 +87,9 @@ __device__ __forceinline__ void flux_face(const R* __restrict__ FSg, R* __restri
     L[q] = FSg[((n * 2 + 1) * 5 + q) * ev + el];
     Rt[q] = FSg[((n * 2 + 0) * 5 + q) * ev + er];
   }
-  roe_flux<R, n, false>(L, Rt, c, F, flags);
+  bool hl = false;
+  roe_flux<R, n, false>(L, Rt, c, F, flags, flags ? &hl : nullptr);
+  if (hl) mark_hlle(g, N, n, i, j, k);
   const int fx = N + di, fy = N + dj;
   const long long nf = (long long)(N + 1) * N * N;
   const long long f = ((long long)k * fy + j) * fx + i;
@@ -112,7 +114,8 @@ __device__ __forceinline__ void flux_face(const R* __restrict__ FSg, R* __restri
 
 template <class R>
 __global__ void __launch_bounds__(128) flux_kernel(const R* __restrict__ FS, R* __restrict__ FL, R* __restrict__ bflux,
-                                                   GenericShape sh, GasConst<R> c, int flags, R* __restrict__ midflux) {
+                                                   GenericShape sh, GasConst<R> c, int flags, R* __restrict__ midflux,
+                                                   long long g0) {
   const int N = sh.N;
   const long long nf = (long long)(N + 1) * N * N;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -125,9 +128,10 @@ __global__ void __launch_bounds__(128) flux_kernel(const R* __restrict__ FS, R* 
   R* mf = midflux ? midflux + (long long)blockIdx.y * 15 * N * N : nullptr;
   const int fx = N + (n == 0), fy = N + (n == 1);
   const int i = (int)(f % fx), j = (int)((f / fx) % fy), k = (int)(f / ((long long)fx * fy));
-  if (n == 0) flux_face<R, 0>(FSg, FLg, bf, sh, c, i, j, k, flags, mf);
-  else if (n == 1) flux_face<R, 1>(FSg, FLg, bf, sh, c, i, j, k, flags, mf);
-  else flux_face<R, 2>(FSg, FLg, bf, sh, c, i, j, k, flags, mf);
+  const long long g = g0 + blockIdx.y;
+  if (n == 0) flux_face<R, 0>(FSg, FLg, bf, sh, c, i, j, k, flags, mf, g);
+  else if (n == 1) flux_face<R, 1>(FSg, FLg, bf, sh, c, i, j, k, flags, mf, g);
+  else flux_face<R, 2>(FSg, FLg, bf, sh, c, i, j, k, flags, mf, g);
 }
 
 template <class R>

@@ -18,6 +18,15 @@ __device__ __forceinline__ void mark_guard(long long g, int N, int i, int j, int
   if (m) m[((g * (N + 2) + (k + 1)) * (N + 2) + (j + 1)) * (N + 2) + (i + 1)] = 1;
 }
 
+// The same for the HLLE fallback of the variant kernels (gamer_hydro_set_hlle_map): when non-null,
+// a face that took the HLLE branch is marked in map[g][n][k][j][i], (N+1)^3 bytes per axis n, the face being the one on
+// the lower side of cell (i, j, k) along n. Read on the fallback path only.
+__device__ unsigned char* gh_hlle_map = nullptr;
+__device__ __forceinline__ void mark_hlle(long long g, int N, int n, int i, int j, int k) {
+  unsigned char* m = gh_hlle_map;
+  if (m) m[(((g * 3 + n) * (N + 1) + k) * (N + 1) + j) * (N + 1) + i] = 1;
+}
+
 template <class R>
 struct GasConst {
   R gamma;      // ratio of specific heats
@@ -177,7 +186,8 @@ __device__ __forceinline__ bool predict_cell(const R Wc[5], const R Wm[3][5], co
 // folds away): plain Roe, no entropy fix. Bit 0: Harten-Hyman entropy fix; bit 1: HLLE fallback when an intermediate
 // state of the linearisation is non-physical (readings R8b / R8c).
 template <class R, int n, bool Fast>
-__device__ __forceinline__ void roe_flux(const R L[5], const R Rt[5], const GasConst<R>& c, R F[5], int flags = 0) {
+__device__ __forceinline__ void roe_flux(const R L[5], const R Rt[5], const GasConst<R>& c, R F[5], int flags = 0,
+                                         bool* took_hlle = nullptr) {
   constexpr int t1 = (n + 1) % 3, t2 = (n + 2) % 3;
   const R uL = L[1 + n], vL = L[1 + t1], wL = L[1 + t2];
   const R uR = Rt[1 + n], vR = Rt[1 + t1], wR = Rt[1 + t2];
@@ -219,6 +229,7 @@ __device__ __forceinline__ void roe_flux(const R L[5], const R Rt[5], const GasC
       F[1 + t1] = ((bp * (mL * vL) - bm * (mR * vR)) + bb * (Rt[0] * vR - L[0] * vL)) * inv_b;
       F[1 + t2] = ((bp * (mL * wL) - bm * (mR * wR)) + bb * (Rt[0] * wR - L[0] * wL)) * inv_b;
       F[4] = ((bp * (mL * HL) - bm * (mR * HR)) + bb * (ER - EL)) * inv_b;
+      if (took_hlle) *took_hlle = true;
       return;
     }
     if (flags & 1) {

@@ -240,3 +240,29 @@ def test_midplane_fluxes_balance_each_half_of_a_group(limiter):
     r0 = O.step_groups(g, 16, 2, dt, dx, G53, 0)
     r1, _ = O.step_groups_ex(g, 16, 2, dt, dx, G53, 0)
     assert np.array_equal(r0.U_out, r1.U_out) and np.array_equal(r0.bflux, r1.bflux)
+
+
+def test_hlle_face_map_marks_exactly_the_faces_whose_flux_changed():
+    """Pin of the diagnostic map step_groups_ex(want_hlle=True) returns (the parity harness' face-level accounting of the
+    HLLE switch rests on its layout [g][axis][k][j][i], face on the lower side of cell (i, j, k)): no face is marked
+    without the flag; with it, a cell none of whose six faces is marked is updated bit for bit as by plain Roe, a cell
+    next to a marked face generally is not; and the marked outer faces are exactly those whose boundary flux changed."""
+    import numpy as np
+    from harness import workloads as wl
+    g = wl.random_groups(2, seed=302, mach=2.0, contrast=0.8)
+    dt, dx, gam = 5e-4, 1 / 16, 5.0 / 3.0
+    r0, _ = O.step_groups_ex(g, 16, 2, dt, dx, gam, 1, 0, want_hlle=True)
+    r2, _ = O.step_groups_ex(g, 16, 2, dt, dx, gam, 1, 2, want_hlle=True)
+    assert r0.hlle.sum() == 0 and r2.hlle.sum() > 1000
+    h = r2.hlle != 0
+    for absent in (h[:, 0, 16], h[:, 0, :, 16], h[:, 1, 16], h[:, 1, :, :, 16], h[:, 2, :, 16], h[:, 2, :, :, 16]):
+        assert not absent.any()                                                    # faces that do not exist stay 0
+    hx, hy, hz = h[:, 0, :16, :16, :], h[:, 1, :16, :, :16], h[:, 2, :, :16, :16]
+    touched = (hx[..., :16] | hx[..., 1:]) | (hy[:, :, :16, :] | hy[:, :, 1:, :]) | (hz[:, :16] | hz[:, 1:])
+    same = np.all(r0.U_out == r2.U_out, axis=1)
+    assert same[~touched].all()                                                    # untouched cells: plain Roe bits
+    assert (~same[touched]).mean() > 0.9                                           # touched cells: the flux changed
+    outer = [hx[..., 0], hx[..., 16], hy[:, :, 0, :], hy[:, :, 16, :], hz[:, 0], hz[:, 16]]
+    for f in range(6):
+        changed = np.any(r0.bflux[:, f] != r2.bflux[:, f], axis=1)
+        assert not changed[~outer[f]].any() and changed[outer[f]].mean() > 0.9
